@@ -1,0 +1,128 @@
+/*
+ * cdh.h -- C ABI of the B200-native particle-pair distance histogram library (libcdh.so).
+ *
+ * What the library computes is the hot path of Reuter & Koefinger, "CADISHI" (arxiv 1808.01478;
+ * citations are PAPER.md:<line> of /root/reference/PAPER.md):
+ *   - Algorithm 1 (section 2.2): for every particle i of species p and j of species q,
+ *     distance vector, minimum image (periodic boxes), r = sqrt(x^2+y^2+z^2),
+ *     kappa = (int) n_bins * r / r_max, ++hist[kappa];
+ *   - one species (p == q): unique pairs j > i only, N(N-1)/2 of them;
+ *   - half-open bins r_kappa <= r < r_kappa + dr (Eq. 4);
+ *   - minimum image dx' = dx - b nint(b^-1 dx) (Eq. 5); b diagonal for an
+ *     orthorhombic box; for a triclinic box dx' is additionally shifted to the 26
+ *     neighbouring cells and the minimum taken (section 2.3);
+ *   - one call takes the whole contiguous multi-species coordinate set and returns ALL species-pair
+ *     histograms; counts are 32 bit inside the kernels and 64 bit in the result
+ *     (PAPER.md:161, 205); histograms of all frames of the call are summed (Eq. 2);
+ *   - device scratch is allocated at the first call and reused.
+ * The per-pair IEEE-754 operation sequence ("pinned sequence") the integers are defined by is stated
+ * in DESIGN.md; the kernels reproduce it bit for bit.
+ *
+ * Threading: one context per device, not thread-safe; a context must not be used on two streams
+ * concurrently.  No call prints, throws or aborts.
+ */
+#ifndef CDH_H
+#define CDH_H
+
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+/* box_type */
+#define CDH_BOX_NONE       0   /* no periodic box */
+#define CDH_BOX_ORTHO      1   /* orthorhombic periodic box (b diagonal) */
+#define CDH_BOX_TRICLINIC  2   /* general triclinic periodic box (Eq. 5 + neighbour shift) */
+
+/* precision */
+#define CDH_F32 0              /* the pinned fp32 sequence (built) */
+#define CDH_F64 1              /* SURVEY.md 8(f) "next": returns CDH_ERR_UNSUPPORTED */
+
+/* return codes */
+#define CDH_OK                 0
+#define CDH_ERR_INVALID_ARG  (-1)  /* detected before anything is enqueued; out untouched */
+#define CDH_ERR_UNSUPPORTED  (-2)
+#define CDH_ERR_ALLOC        (-3)  /* device or pinned-host allocation failed */
+#define CDH_ERR_CUDA         (-4)  /* a CUDA runtime call failed; text via cdh_last_error() */
+
+/* cdh_create flags: 0 for production.  The other bits force a kernel variant (tests, ncu A/B runs);
+ * every variant returns the same integers. */
+#define CDH_FLAG_SIMPLE_KERNEL   (1u << 0) /* plain scalar kernel with library sqrtf/rintf/floorf: the
+                                              cross-validation kernel */
+#define CDH_FLAG_NO_PRUNE        (1u << 1) /* triclinic: always search the 27 shifts */
+#define CDH_FLAG_WARP_AGGREGATE  (1u << 2) /* always aggregate equal bins in a warp (__match_any_sync) */
+#define CDH_FLAG_NO_AGGREGATE    (1u << 3) /* never aggregate */
+#define CDH_FLAG_MAX_SMEM_BINS_SHIFT 8     /* bits 8..31: if non-zero, cap on the bins one CTA keeps in
+                                              shared memory (forces the bin-range-split path) */
+
+typedef struct cdh_ctx cdh_ctx;  /* opaque; owns device scratch (repacked coordinates, work tables) only */
+
+/* Create a context on CUDA device `device` (HOST call; selects the device for the calling thread while
+ * it runs and restores the previous one).  *ctx receives the context.  Returns CDH_OK,
+ * CDH_ERR_INVALID_ARG (ctx NULL, no such device, not an sm_100 device), CDH_ERR_ALLOC, CDH_ERR_CUDA. */
+int cdh_create(cdh_ctx **ctx, int device, uint32_t flags);
+
+/*
+ * All species-pair histograms of n_frames frames, summed over the frames.
+ *
+ *  coords          DEVICE pointer, [n_frames][n_total][3] xyz AoS, contiguous, float (precision CDH_F32).
+ *                  Coordinates need not be wrapped into the box.  Pairs involving a NaN are dropped.
+ *                  Read only during the stream-ordered execution of the call.
+ *  n_frames        >= 1.
+ *  species_offsets HOST pointer, [n_species + 1]; [0] == 0, non-decreasing, [n_species] == n_total < 2^31;
+ *                  the same for every frame.  Empty species are legal (zero histograms).
+ *  n_species       >= 1.
+ *  box_type        CDH_BOX_*.
+ *  box             HOST pointer, [n_boxes][9] row-major doubles, ROWS are the box vectors a, b, c
+ *                  (the mathematical b of Eq. 5 has them as columns); NULL iff CDH_BOX_NONE.
+ *                  CDH_BOX_ORTHO reads the diagonal and requires the off-diagonals to be exactly 0.
+ *                  Must be finite and non-singular.
+ *  n_boxes         1 (one box for all frames) or n_frames; ignored for CDH_BOX_NONE.
+ *  r_max           > 0, finite.  Pairs with !(r < (float)r_max) are dropped in every box mode.
+ *  n_bins          1 .. 2^22.  Bin width r_max / n_bins; bin = floor(r * (float)(n_bins / r_max)),
+ *                  a kept pair whose product rounds up to n_bins goes to bin n_bins - 1.
+ *  precision       CDH_F32.
+ *  stream          cudaStream_t (as void*), may be 0.  All work is enqueued on it; the call does not
+ *                  synchronise.  `out` is valid once the caller has synchronised the stream.
+ *  out             DEVICE pointer, uint64 [n_species*(n_species+1)/2][n_bins], OVERWRITTEN.
+ *                  Row index of species pair (p <= q): p*n_species - p*(p-1)/2 + (q - p).
+ *
+ * Host arrays are read during the call only.  Returns CDH_OK or a negative code; on
+ * CDH_ERR_INVALID_ARG nothing was enqueued.
+ */
+int cdh_histograms(cdh_ctx *ctx, const void *coords, int32_t n_frames,
+                   const int32_t *species_offsets, int32_t n_species, int32_t box_type,
+                   const double *box, int32_t n_boxes, double r_max, int32_t n_bins,
+                   int32_t precision, void *stream, uint64_t *out);
+
+/* Same computation with HOST buffers: `coords` and `out` are host pointers (pageable or pinned).  The
+ * library copies the coordinates to the device (one H2D copy), runs cdh_histograms on
+ * `stream`, copies the result back (one D2H copy) and SYNCHRONISES the stream before returning.
+ * Other arguments, return codes and error behaviour as cdh_histograms. */
+int cdh_histograms_host(cdh_ctx *ctx, const void *coords, int32_t n_frames,
+                        const int32_t *species_offsets, int32_t n_species, int32_t box_type,
+                        const double *box, int32_t n_boxes, double r_max, int32_t n_bins,
+                        int32_t precision, void *stream, uint64_t *out);
+
+/* Destroy the context and free its scratch (synchronises the device).  NULL is accepted. */
+int cdh_destroy(cdh_ctx *ctx);
+
+/* Static text for a return code. */
+const char *cdh_strerror(int code);
+
+/* Text of the last CUDA error recorded by this context ("" if none); valid until the next call on ctx. */
+const char *cdh_last_error(const cdh_ctx *ctx);
+
+/* Introspection of the LAST cdh_histograms call on ctx (host values, no synchronisation):
+ *   info[0] = kernels launched by the call      info[1] = work items (tile pairs) scheduled
+ *   info[2] = bin-range sweeps                   info[3] = CTAs of the tile kernel
+ *   info[4] = threads per CTA                    info[5] = dynamic shared memory bytes per CTA
+ *   info[6] = kernel variant id                  info[7] = evaluated pairs incl. padding lanes (low 32 bits unused; see info64)
+ * Returns CDH_OK or CDH_ERR_INVALID_ARG. */
+int cdh_last_call_info(const cdh_ctx *ctx, int64_t info[8]);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* CDH_H */
