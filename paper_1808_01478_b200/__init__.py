@@ -1,0 +1,24 @@
+"""paper_1808_01478_b200 -- B200-native particle-pair distance histograms (CADISHI hot path).
+
+The product is ``libcdh.so`` (C ABI in ``include/cdh.h``, CUDA kernels in ``csrc/``); this package is
+its thin Python binding plus the seeded input generators (``inputs``).  Importing the package does not
+load the library; the first call does, and fails loudly if it was not built.
+"""
+from . import inputs  # noqa: F401
+from .binding import (BOX_NONE, BOX_ORTHO, BOX_TRICLINIC, F32, F64, FLAG_MAX_SMEM_BINS_SHIFT,  # noqa: F401
+                      FLAG_NO_AGGREGATE, FLAG_NO_PRUNE, FLAG_SIMPLE_KERNEL, FLAG_WARP_AGGREGATE, CdhError,
+                      Context, cdh_bench_fp32_rate, cdh_bench_shared_atomics, cdh_create, cdh_selftest_sqrt,
+                      cdh_strerror, load)
+
+
+def histograms_device(ctx: "Context", problem, stream=None):
+    """Run ``cdh_histograms`` on an ``inputs.Problem``: copies the coordinates to the context's device
+    with torch (plumbing), calls the library, returns a torch uint64-as-int64 CUDA tensor [n_hist, n_bins]
+    (not synchronised)."""
+    import torch
+    dev = torch.device("cuda", ctx.device)
+    coords = torch.from_numpy(problem.coords).to(dev)
+    out = torch.empty((problem.n_hist, problem.n_bins), dtype=torch.int64, device=dev)
+    ctx.cdh_histograms(coords, problem.n_frames, problem.species_offsets, problem.box_type, problem.box,
+                       problem.r_max, problem.n_bins, out, stream=stream)
+    return out

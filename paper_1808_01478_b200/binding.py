@@ -1,0 +1,225 @@
+"""ctypes binding of libcdh.so: same names as include/cdh.h, argument marshalling only.
+
+Every step of the path runs inside the CUDA library; there is no CPU fallback.  Loading or calling
+without the built library / without a CUDA device raises (``CdhError`` or ``OSError``).
+PyTorch is used by callers for device buffers and streams only; this module accepts torch CUDA
+tensors or raw device pointers (ints).
+"""
+from __future__ import annotations
+
+import ctypes
+import os
+from typing import Optional, Sequence
+
+import numpy as np
+
+_HERE = os.path.dirname(os.path.abspath(__file__))
+LIB_PATH = os.path.join(_HERE, "libcdh.so")
+
+BOX_NONE, BOX_ORTHO, BOX_TRICLINIC = 0, 1, 2
+F32, F64 = 0, 1
+OK, ERR_INVALID_ARG, ERR_UNSUPPORTED, ERR_ALLOC, ERR_CUDA = 0, -1, -2, -3, -4
+FLAG_SIMPLE_KERNEL = 1 << 0
+FLAG_NO_PRUNE = 1 << 1
+FLAG_WARP_AGGREGATE = 1 << 2
+FLAG_NO_AGGREGATE = 1 << 3
+FLAG_MAX_SMEM_BINS_SHIFT = 8
+
+EXPORTS = ["cdh_create", "cdh_histograms", "cdh_histograms_host", "cdh_destroy", "cdh_strerror",
+           "cdh_last_error", "cdh_last_call_info",
+           "cdh_bench_fp32_rate", "cdh_bench_shared_atomics", "cdh_selftest_sqrt"]
+
+
+class CdhError(RuntimeError):
+    def __init__(self, code: int, text: str):
+        super().__init__(f"cdh error {code}: {text}")
+        self.code = code
+
+
+_lib = None
+
+
+def load(path: Optional[str] = None) -> ctypes.CDLL:
+    """dlopen libcdh.so and declare the signatures.  Fails loudly if it was not built."""
+    global _lib
+    if _lib is not None and path is None:
+        return _lib
+    p = path or LIB_PATH
+    if not os.path.exists(p):
+        raise OSError(f"{p} not found: build it with `python -m paper_1808_01478_b200.build` "
+                      "(there is no CPU fallback)")
+    lib = ctypes.CDLL(p)
+    vp, i32, u32, dbl = ctypes.c_void_p, ctypes.c_int32, ctypes.c_uint32, ctypes.c_double
+    lib.cdh_create.restype = ctypes.c_int
+    lib.cdh_create.argtypes = [ctypes.POINTER(vp), ctypes.c_int, u32]
+    hist_args = [vp, vp, i32, vp, i32, i32, vp, i32, dbl, i32, i32, vp, vp]
+    lib.cdh_histograms.restype = ctypes.c_int
+    lib.cdh_histograms.argtypes = hist_args
+    lib.cdh_histograms_host.restype = ctypes.c_int
+    lib.cdh_histograms_host.argtypes = hist_args
+    lib.cdh_destroy.restype = ctypes.c_int
+    lib.cdh_destroy.argtypes = [vp]
+    lib.cdh_strerror.restype = ctypes.c_char_p
+    lib.cdh_strerror.argtypes = [ctypes.c_int]
+    lib.cdh_last_error.restype = ctypes.c_char_p
+    lib.cdh_last_error.argtypes = [vp]
+    lib.cdh_last_call_info.restype = ctypes.c_int
+    lib.cdh_last_call_info.argtypes = [vp, ctypes.POINTER(ctypes.c_int64)]
+    lib.cdh_bench_fp32_rate.restype = ctypes.c_int
+    lib.cdh_bench_fp32_rate.argtypes = [ctypes.c_int, ctypes.c_int, vp, ctypes.POINTER(dbl), ctypes.POINTER(dbl)]
+    lib.cdh_bench_shared_atomics.restype = ctypes.c_int
+    lib.cdh_bench_shared_atomics.argtypes = [ctypes.c_int, ctypes.c_int, ctypes.c_int, vp, ctypes.c_int, dbl,
+                                             ctypes.c_int, ctypes.c_int, ctypes.c_int, vp,
+                                             ctypes.POINTER(dbl), ctypes.POINTER(dbl), ctypes.POINTER(dbl)]
+    lib.cdh_selftest_sqrt.restype = ctypes.c_int
+    lib.cdh_selftest_sqrt.argtypes = [u32, u32, vp, ctypes.POINTER(ctypes.c_uint64)]
+    if path is None:
+        _lib = lib
+    return lib
+
+
+def cdh_strerror(code: int) -> str:
+    return load().cdh_strerror(int(code)).decode()
+
+
+def _ptr(x) -> int:
+    """Device/host address of a torch tensor, numpy array or int."""
+    if x is None:
+        return 0
+    if isinstance(x, int):
+        return x
+    if hasattr(x, "data_ptr"):
+        return int(x.data_ptr())
+    if isinstance(x, np.ndarray):
+        return int(x.ctypes.data)
+    raise TypeError(f"cannot take the address of {type(x)}")
+
+
+def _stream_ptr(stream) -> int:
+    if stream is None:
+        return 0
+    if isinstance(stream, int):
+        return stream
+    return int(stream.cuda_stream)          # torch.cuda.Stream
+
+
+class Context:
+    """Owns one ``cdh_ctx`` (device scratch).  One per device; not thread-safe."""
+
+    def __init__(self, device: int = 0, flags: int = 0):
+        self._lib = load()
+        h = ctypes.c_void_p()
+        rc = self._lib.cdh_create(ctypes.byref(h), int(device), int(flags))
+        if rc != OK:
+            raise CdhError(rc, cdh_strerror(rc))
+        self._h = h
+        self.device = int(device)
+
+    def _check(self, rc: int):
+        if rc != OK:
+            detail = self._lib.cdh_last_error(self._h).decode() if self._h else ""
+            raise CdhError(rc, cdh_strerror(rc) + (f" [{detail}]" if detail else ""))
+
+    def _marshal(self, species_offsets, box, n_frames):
+        off = np.ascontiguousarray(species_offsets, dtype=np.int32)
+        if box is None:
+            b, n_boxes = None, 0
+        else:
+            b = np.ascontiguousarray(box, dtype=np.float64).reshape(-1, 9)
+            n_boxes = int(b.shape[0])
+        return off, b, n_boxes
+
+    def cdh_histograms(self, coords, n_frames: int, species_offsets: Sequence[int], box_type: int,
+                       box, r_max: float, n_bins: int, out, precision: int = F32, stream=None) -> None:
+        """include/cdh.h ``cdh_histograms``: coords / out are DEVICE buffers (torch CUDA tensors or ints).
+        Asynchronous on ``stream``."""
+        off, b, n_boxes = self._marshal(species_offsets, box, n_frames)
+        rc = self._lib.cdh_histograms(self._h, _ptr(coords), int(n_frames), off.ctypes.data, len(off) - 1,
+                                      int(box_type), None if b is None else b.ctypes.data, n_boxes,
+                                      float(r_max), int(n_bins), int(precision), _stream_ptr(stream), _ptr(out))
+        self._check(rc)
+
+    def cdh_histograms_host(self, coords: np.ndarray, species_offsets: Sequence[int], box_type: int, box,
+                            r_max: float, n_bins: int, precision: int = F32, stream=None,
+                            out: Optional[np.ndarray] = None) -> np.ndarray:
+        """include/cdh.h ``cdh_histograms_host``: HOST numpy coords [n_frames, n_total, 3] -> HOST uint64
+        [n_hist, n_bins]; H2D, kernels and D2H inside the call; synchronises ``stream``."""
+        c = np.ascontiguousarray(coords)
+        if c.ndim == 2:
+            c = c[None]
+        if c.dtype != np.float32 or c.ndim != 3 or c.shape[2] != 3:
+            raise ValueError("coords must be float32 [n_frames, n_total, 3]")
+        off, b, n_boxes = self._marshal(species_offsets, box, c.shape[0])
+        n_species = len(off) - 1
+        n_hist = n_species * (n_species + 1) // 2
+        if out is None:
+            out = np.empty((n_hist, int(n_bins)), dtype=np.uint64)
+        rc = self._lib.cdh_histograms_host(self._h, c.ctypes.data, int(c.shape[0]), off.ctypes.data, n_species,
+                                           int(box_type), None if b is None else b.ctypes.data, n_boxes,
+                                           float(r_max), int(n_bins), int(precision), _stream_ptr(stream),
+                                           out.ctypes.data)
+        self._check(rc)
+        return out
+
+    def last_call_info(self) -> dict:
+        arr = (ctypes.c_int64 * 8)()
+        self._check(self._lib.cdh_last_call_info(self._h, arr))
+        v = list(arr)
+        return {"launches": v[0], "items": v[1], "sweeps": v[2], "ctas": v[3], "threads": v[4],
+                "smem_bytes": v[5], "variant": v[6], "tj": v[6] >> 16, "fast": bool(v[6] & 1),
+                "padded_pairs": v[7]}
+
+    def cdh_destroy(self) -> None:
+        if self._h:
+            self._lib.cdh_destroy(self._h)
+            self._h = None
+
+    close = cdh_destroy
+
+    def __enter__(self):
+        return self
+
+    def __exit__(self, *exc):
+        self.cdh_destroy()
+
+    def __del__(self):
+        try:
+            self.cdh_destroy()
+        except Exception:
+            pass
+
+
+def cdh_create(device: int = 0, flags: int = 0) -> Context:
+    return Context(device, flags)
+
+
+# ---- microbenchmarks (include/cdh_bench.h) ---------------------------------------------------------
+def cdh_bench_fp32_rate(kind: int, iters: int = 2048, stream=None):
+    lib = load()
+    r, ms = ctypes.c_double(), ctypes.c_double()
+    rc = lib.cdh_bench_fp32_rate(int(kind), int(iters), _stream_ptr(stream), ctypes.byref(r), ctypes.byref(ms))
+    if rc != OK:
+        raise CdhError(rc, cdh_strerror(rc))
+    return r.value, ms.value
+
+
+def cdh_bench_shared_atomics(pattern: int, op: int, n_bins: int, samples=None, n_samples: int = 0,
+                             active_fraction: float = 1.0, threads: int = 512, ctas_per_sm: int = 1,
+                             iters: int = 4096, stream=None):
+    lib = load()
+    r, ms, ms0 = ctypes.c_double(), ctypes.c_double(), ctypes.c_double()
+    rc = lib.cdh_bench_shared_atomics(int(pattern), int(op), int(n_bins), _ptr(samples), int(n_samples),
+                                      float(active_fraction), int(threads), int(ctas_per_sm), int(iters),
+                                      _stream_ptr(stream), ctypes.byref(r), ctypes.byref(ms), ctypes.byref(ms0))
+    if rc != OK:
+        raise CdhError(rc, cdh_strerror(rc))
+    return r.value, ms.value, ms0.value
+
+
+def cdh_selftest_sqrt(first_bits: int = 0x0D000000, last_bits: int = 0x7F7FFFFF, stream=None) -> int:
+    lib = load()
+    bad = ctypes.c_uint64()
+    rc = lib.cdh_selftest_sqrt(int(first_bits), int(last_bits), _stream_ptr(stream), ctypes.byref(bad))
+    if rc != OK:
+        raise CdhError(rc, cdh_strerror(rc))
+    return int(bad.value)

@@ -1,0 +1,51 @@
+"""Build libcdh.so (the C-ABI CUDA library) in-tree with nvcc for sm_100a.
+
+``python -m paper_1808_01478_b200.build`` or ``build()``; nvcc cross-compiles without a GPU.
+The host code derives constants of the pinned sequence in double, so it is compiled without FP
+contraction (-ffp-contract=off).
+"""
+from __future__ import annotations
+
+import os
+import subprocess
+import sys
+
+_HERE = os.path.dirname(os.path.abspath(__file__))
+CSRC = os.path.join(_HERE, "csrc")
+LIB = os.path.join(_HERE, "libcdh.so")
+SOURCES = ["cdh_api.cu", "cdh_bench.cu"]
+DEPS = SOURCES + ["cdh_device.cuh", "cdh_kernels.cuh", "cdh_fast.cuh", "cdh_tile.cuh", "cdh_host.h",
+                  os.path.join("..", "..", "include", "cdh.h"), os.path.join("..", "..", "include", "cdh_bench.h")]
+NVCC_FLAGS = ["-gencode", "arch=compute_100a,code=sm_100a", "-O3", "-lineinfo", "-std=c++17",
+              "-Xcompiler", "-fPIC,-ffp-contract=off,-fno-fast-math", "-shared", "-cudart", "static"]
+
+
+def nvcc_path() -> str:
+    for cand in (os.environ.get("NVCC"), "/usr/local/cuda/bin/nvcc", "nvcc"):
+        if cand and (os.path.isabs(cand) and os.path.exists(cand) or not os.path.isabs(cand)):
+            return cand
+    return "nvcc"
+
+
+def is_stale() -> bool:
+    if not os.path.exists(LIB):
+        return True
+    t = os.path.getmtime(LIB)
+    return any(os.path.getmtime(os.path.join(CSRC, d)) > t for d in DEPS)
+
+
+def build(force: bool = False, verbose: bool = False) -> str:
+    """Compile if the library is missing or older than a source; returns its path."""
+    if force or is_stale():
+        tmp = LIB + f".tmp{os.getpid()}"
+        cmd = [nvcc_path(), *NVCC_FLAGS, "-o", tmp, *[os.path.join(CSRC, s) for s in SOURCES]]
+        if verbose:
+            cmd.insert(1, "-Xptxas=-v")
+            print(" ".join(cmd), file=sys.stderr)
+        subprocess.run(cmd, check=True, cwd=CSRC)
+        os.replace(tmp, LIB)
+    return LIB
+
+
+if __name__ == "__main__":
+    print(build(force="--force" in sys.argv, verbose="-v" in sys.argv))

@@ -1,0 +1,328 @@
+// cdh_api.cu -- the C ABI of libcdh (include/cdh.h): context, validation, host dispatch.
+// All device work of a call is enqueued on the caller's stream; cdh_histograms never synchronises.
+#include <cstdio>
+#include <new>
+#include <string>
+#include "cdh_host.h"
+#include "cdh_tile.cuh"
+
+using namespace cdh;
+
+struct cdh_ctx {
+    int device = 0;
+    uint32_t flags = 0;
+    int n_sm = 0;
+    int max_smem_optin = 0;
+    // device scratch, grown on demand, never shrunk
+    float* d_pk = nullptr;       size_t pk_bytes = 0;
+    void* d_tables = nullptr;    size_t tables_bytes = 0;     // segs | rows | boxes | off | pad_off
+    unsigned int* d_scalars = nullptr;                        // [0] work counter (fast), [1] extent bits, [2] counter (simple)
+    void* h_tables = nullptr;    size_t h_tables_bytes = 0;   // pinned staging for d_tables
+    cudaEvent_t staged = nullptr;                             // h_tables may be rewritten once this has fired
+    bool staged_pending = false;
+    void* d_io_coords = nullptr; size_t io_coords_bytes = 0;  // cdh_histograms_host staging
+    void* d_io_out = nullptr;    size_t io_out_bytes = 0;
+    std::string err;
+    int64_t info[8] = {0, 0, 0, 0, 0, 0, 0, 0};
+};
+
+namespace {
+
+struct DeviceGuard {
+    int prev = -1; bool ok;
+    explicit DeviceGuard(int dev) { ok = cudaGetDevice(&prev) == cudaSuccess && cudaSetDevice(dev) == cudaSuccess; }
+    ~DeviceGuard() { if (prev >= 0) cudaSetDevice(prev); }
+};
+
+int cuda_fail(cdh_ctx* c, cudaError_t e, const char* what) {
+    c->err = std::string(what) + ": " + cudaGetErrorString(e);
+    return CDH_ERR_CUDA;
+}
+#define CDH_CUDA(call)                                                       \
+    do { cudaError_t e_ = (call); if (e_ != cudaSuccess) return cuda_fail(ctx, e_, #call); } while (0)
+
+int grow(cdh_ctx* ctx, void** p, size_t* have, size_t need, bool pinned_host) {
+    if (need <= *have) return CDH_OK;
+    if (*p) {
+        // a buffer still in use by enqueued work must not be freed under it
+        cudaError_t e = cudaDeviceSynchronize();
+        if (e != cudaSuccess) return cuda_fail(ctx, e, "cudaDeviceSynchronize");
+        if (pinned_host) cudaFreeHost(*p); else cudaFree(*p);
+        *p = nullptr; *have = 0;
+    }
+    const size_t want = need + need / 4 + 4096;
+    cudaError_t e = pinned_host ? cudaMallocHost(p, want) : cudaMalloc(p, want);
+    if (e != cudaSuccess) { cudaGetLastError(); *p = nullptr; ctx->err = cudaGetErrorString(e); return CDH_ERR_ALLOC; }
+    *have = want;
+    return CDH_OK;
+}
+
+// ---- kernel table -----------------------------------------------------------------------------
+typedef void (*TileFn)(const TileParams);
+struct Variant { TileFn fn; int threads; };
+
+template <int BOX, int TRI, bool SPLIT>
+Variant fast_variant(bool big) {
+    if (big) return {tile_kernel<BOX, TRI, 512, VAR_FAST, SPLIT, 1>, 512};
+    return {tile_kernel<BOX, TRI, 256, VAR_FAST, SPLIT, 2>, 256};
+}
+template <bool SPLIT>
+Variant pick_fast(int box_type, int tri, bool big) {
+    if (box_type == CDH_BOX_NONE) return fast_variant<BOX_NONE, 0, SPLIT>(big);
+    if (box_type == CDH_BOX_ORTHO) return fast_variant<BOX_ORTHO, 0, SPLIT>(big);
+    if (tri == TRI_UPPER_B01) return fast_variant<BOX_TRI, TRI_UPPER_B01, SPLIT>(big);
+    if (tri == TRI_UPPER) return fast_variant<BOX_TRI, TRI_UPPER, SPLIT>(big);
+    return fast_variant<BOX_TRI, TRI_GENERAL, SPLIT>(big);
+}
+Variant pick_simple(int box_type, bool big) {
+    if (box_type == CDH_BOX_NONE)
+        return big ? Variant{tile_kernel<BOX_NONE, 0, 512, VAR_SIMPLE, true, 1>, 512} : Variant{tile_kernel<BOX_NONE, 0, 256, VAR_SIMPLE, true, 2>, 256};
+    if (box_type == CDH_BOX_ORTHO)
+        return big ? Variant{tile_kernel<BOX_ORTHO, 0, 512, VAR_SIMPLE, true, 1>, 512} : Variant{tile_kernel<BOX_ORTHO, 0, 256, VAR_SIMPLE, true, 2>, 256};
+    return big ? Variant{tile_kernel<BOX_TRI, 0, 512, VAR_SIMPLE, true, 1>, 512} : Variant{tile_kernel<BOX_TRI, 0, 256, VAR_SIMPLE, true, 2>, 256};
+}
+
+}  // namespace
+
+extern "C" const char* cdh_strerror(int code) {
+    switch (code) {
+        case CDH_OK: return "ok";
+        case CDH_ERR_INVALID_ARG: return "invalid argument";
+        case CDH_ERR_UNSUPPORTED: return "unsupported (precision CDH_F64 is not built)";
+        case CDH_ERR_ALLOC: return "allocation failed";
+        case CDH_ERR_CUDA: return "CUDA runtime error (see cdh_last_error)";
+        default: return "unknown error code";
+    }
+}
+
+extern "C" const char* cdh_last_error(const cdh_ctx* ctx) { return ctx ? ctx->err.c_str() : ""; }
+
+extern "C" int cdh_last_call_info(const cdh_ctx* ctx, int64_t info[8]) {
+    if (!ctx || !info) return CDH_ERR_INVALID_ARG;
+    for (int k = 0; k < 8; ++k) info[k] = ctx->info[k];
+    return CDH_OK;
+}
+
+extern "C" int cdh_create(cdh_ctx** out, int device, uint32_t flags) {
+    if (!out) return CDH_ERR_INVALID_ARG;
+    *out = nullptr;
+    int n_dev = 0;
+    if (cudaGetDeviceCount(&n_dev) != cudaSuccess) { cudaGetLastError(); return CDH_ERR_CUDA; }
+    if (device < 0 || device >= n_dev) return CDH_ERR_INVALID_ARG;
+    cudaDeviceProp prop;
+    if (cudaGetDeviceProperties(&prop, device) != cudaSuccess) { cudaGetLastError(); return CDH_ERR_CUDA; }
+    if (prop.major != 10) return CDH_ERR_INVALID_ARG;            // sm_100a code only
+    cdh_ctx* ctx = new (std::nothrow) cdh_ctx;
+    if (!ctx) return CDH_ERR_ALLOC;
+    ctx->device = device; ctx->flags = flags;
+    ctx->n_sm = prop.multiProcessorCount;
+    ctx->max_smem_optin = (int)prop.sharedMemPerBlockOptin;
+    DeviceGuard g(device);
+    if (!g.ok || cudaMalloc(&ctx->d_scalars, 64) != cudaSuccess ||
+        cudaEventCreateWithFlags(&ctx->staged, cudaEventDisableTiming) != cudaSuccess) {
+        cudaGetLastError();
+        if (ctx->d_scalars) cudaFree(ctx->d_scalars);
+        delete ctx;
+        return CDH_ERR_ALLOC;
+    }
+    *out = ctx;
+    return CDH_OK;
+}
+
+extern "C" int cdh_destroy(cdh_ctx* ctx) {
+    if (!ctx) return CDH_OK;
+    DeviceGuard g(ctx->device);
+    cudaDeviceSynchronize();
+    if (ctx->d_pk) cudaFree(ctx->d_pk);
+    if (ctx->d_tables) cudaFree(ctx->d_tables);
+    if (ctx->d_scalars) cudaFree(ctx->d_scalars);
+    if (ctx->h_tables) cudaFreeHost(ctx->h_tables);
+    if (ctx->d_io_coords) cudaFree(ctx->d_io_coords);
+    if (ctx->d_io_out) cudaFree(ctx->d_io_out);
+    if (ctx->staged) cudaEventDestroy(ctx->staged);
+    cudaGetLastError();
+    delete ctx;
+    return CDH_OK;
+}
+
+static int validate(const void* coords, int32_t n_frames, const int32_t* off, int32_t n_species, int32_t box_type,
+                    const double* box, int32_t n_boxes, double r_max, int32_t n_bins, int32_t precision, const void* out) {
+    if (!coords || !off || !out) return CDH_ERR_INVALID_ARG;
+    if (n_frames < 1 || n_species < 1 || n_species > 4096) return CDH_ERR_INVALID_ARG;
+    if (n_bins < 1 || n_bins > (1 << 22)) return CDH_ERR_INVALID_ARG;
+    if (!(r_max > 0.0) || !std::isfinite(r_max)) return CDH_ERR_INVALID_ARG;
+    if (precision != CDH_F32 && precision != CDH_F64) return CDH_ERR_INVALID_ARG;
+    if (box_type != CDH_BOX_NONE && box_type != CDH_BOX_ORTHO && box_type != CDH_BOX_TRICLINIC) return CDH_ERR_INVALID_ARG;
+    if (box_type == CDH_BOX_NONE ? (box != nullptr) : (box == nullptr)) return CDH_ERR_INVALID_ARG;
+    if (box_type != CDH_BOX_NONE && n_boxes != 1 && n_boxes != n_frames) return CDH_ERR_INVALID_ARG;
+    if (off[0] != 0) return CDH_ERR_INVALID_ARG;
+    for (int s = 0; s < n_species; ++s) if (off[s + 1] < off[s]) return CDH_ERR_INVALID_ARG;
+    if (!((float)r_max > 0.0f) || !std::isfinite((float)r_max)) return CDH_ERR_INVALID_ARG;
+    const float scale = (float)((double)n_bins / r_max);
+    if (!std::isfinite(scale) || !(scale > 0.0f)) return CDH_ERR_INVALID_ARG;
+    if (precision == CDH_F64) return CDH_ERR_UNSUPPORTED;
+    return CDH_OK;
+}
+
+static inline size_t align256(size_t x) { return (x + 255) & ~(size_t)255; }
+
+extern "C" int cdh_histograms(cdh_ctx* ctx, const void* coords, int32_t n_frames, const int32_t* off,
+                              int32_t n_species, int32_t box_type, const double* box, int32_t n_boxes,
+                              double r_max, int32_t n_bins, int32_t precision, void* stream_, uint64_t* out) {
+    if (!ctx) return CDH_ERR_INVALID_ARG;
+    int rc = validate(coords, n_frames, off, n_species, box_type, box, n_boxes, r_max, n_bins, precision, out);
+    if (rc != CDH_OK) return rc;
+    cudaStream_t stream = (cudaStream_t)stream_;
+    ctx->err.clear();
+
+    // ---- host-derived constants ----------------------------------------------------------------
+    const int nb = (box_type == CDH_BOX_NONE) ? 0 : n_boxes;
+    std::vector<BoxConst> boxes((size_t)(nb > 0 ? nb : 1));
+    std::memset(boxes.data(), 0, boxes.size() * sizeof(BoxConst));
+    for (int b = 0; b < nb; ++b) {
+        if (!make_box_const(box_type, box + 9 * (size_t)b, r_max, &boxes[b])) return CDH_ERR_INVALID_ARG;
+        if (ctx->flags & CDH_FLAG_NO_PRUNE) boxes[b].prune_ok = 0.0f;
+    }
+    const int tri = (box_type == CDH_BOX_TRICLINIC) ? tri_kind(boxes.data(), nb) : 0;
+    const float rmax_f = (float)r_max;
+    const float scale_f = (float)((double)n_bins / r_max);
+
+    // ---- padded layout -------------------------------------------------------------------------
+    std::vector<uint32_t> pad_off((size_t)n_species + 1);
+    uint64_t slots = 0;
+    for (int s = 0; s < n_species; ++s) {
+        pad_off[s] = (uint32_t)slots;
+        const uint64_t n = (uint64_t)(off[s + 1] - off[s]);
+        slots += (n + kPadParticles - 1) / kPadParticles * kPadParticles;
+        if (slots > 0x7fffffffull) return CDH_ERR_INVALID_ARG;
+    }
+    pad_off[n_species] = (uint32_t)slots;
+    const uint32_t frame_slots = (uint32_t)slots;
+    if ((uint64_t)frame_slots * (uint64_t)n_frames / kGroup > 0xffffffffull) return CDH_ERR_INVALID_ARG;
+    const int n_hist = n_species * (n_species + 1) / 2;
+
+    DeviceGuard guard(ctx->device);
+    if (!guard.ok) return cuda_fail(ctx, cudaGetLastError(), "cudaSetDevice");
+
+    // ---- variant, sweeps, tile sizes -----------------------------------------------------------
+    uint32_t cap_bins = (uint32_t)((ctx->max_smem_optin - tile_smem_bytes(0)) / 4);
+    const uint32_t flag_cap = ctx->flags >> CDH_FLAG_MAX_SMEM_BINS_SHIFT;
+    if (flag_cap && flag_cap < cap_bins) cap_bins = flag_cap;
+    const SweepPlan sp = plan_sweeps((uint32_t)n_bins, cap_bins);
+    const int smem_bytes = tile_smem_bytes((int)sp.bins_per_sweep);
+    const bool big = 2 * (smem_bytes + 1024) > 228 * 1024;          // one CTA per SM
+    const bool split = sp.n_sweeps > 1;
+    bool use_simple_only = (ctx->flags & CDH_FLAG_SIMPLE_KERNEL) != 0 || !(scale_f < 5.0e14f);
+    const Variant vf = split ? pick_fast<true>(box_type, tri, big) : pick_fast<false>(box_type, tri, big);
+    const Variant vs = pick_simple(box_type, big);
+    const uint32_t ti = (uint32_t)vf.threads * kR;
+    const uint32_t grid_full = (uint32_t)ctx->n_sm * (big ? 1u : 2u);
+
+    WorkTables wt;
+    uint32_t tj = 8192;
+    for (;; tj >>= 1) {
+        build_tables(n_frames, off, n_species, nb > 0 ? nb : 1, (uint32_t)n_bins, sp, ti, tj, pad_off, frame_slots, &wt);
+        if (wt.n_items >= 16ull * grid_full || tj == (uint32_t)kStageParticles) break;
+    }
+    if (wt.n_items >= 0xffffffffull || wt.rows.size() >= 0x7fffffffull) return CDH_ERR_INVALID_ARG;
+
+    // ---- scratch -------------------------------------------------------------------------------
+    const size_t b_segs = align256(wt.segs.size() * sizeof(Seg) + 1), b_rows = align256(wt.rows.size() * sizeof(Row)),
+                 b_boxes = align256(boxes.size() * sizeof(BoxConst)), b_off = align256(((size_t)n_species + 1) * 4);
+    const size_t tables = b_segs + b_rows + b_boxes + 2 * b_off;
+    if (ctx->staged_pending) { CDH_CUDA(cudaEventSynchronize(ctx->staged)); ctx->staged_pending = false; }
+    if ((rc = grow(ctx, &ctx->h_tables, &ctx->h_tables_bytes, tables, true)) != CDH_OK) return rc;
+    if ((rc = grow(ctx, &ctx->d_tables, &ctx->tables_bytes, tables, false)) != CDH_OK) return rc;
+    const size_t pk_need = (size_t)n_frames * frame_slots * 3 * sizeof(float);
+    if ((rc = grow(ctx, (void**)&ctx->d_pk, &ctx->pk_bytes, pk_need > 0 ? pk_need : 16, false)) != CDH_OK) return rc;
+
+    char* h = (char*)ctx->h_tables;
+    std::memcpy(h, wt.segs.data(), wt.segs.size() * sizeof(Seg));
+    std::memcpy(h + b_segs, wt.rows.data(), wt.rows.size() * sizeof(Row));
+    std::memcpy(h + b_segs + b_rows, boxes.data(), boxes.size() * sizeof(BoxConst));
+    std::memcpy(h + b_segs + b_rows + b_boxes, off, ((size_t)n_species + 1) * 4);
+    std::memcpy(h + b_segs + b_rows + b_boxes + b_off, pad_off.data(), ((size_t)n_species + 1) * 4);
+    char* d = (char*)ctx->d_tables;
+    CDH_CUDA(cudaMemcpyAsync(d, h, tables, cudaMemcpyHostToDevice, stream));
+    CDH_CUDA(cudaEventRecord(ctx->staged, stream));
+    ctx->staged_pending = true;
+    CDH_CUDA(cudaMemsetAsync(ctx->d_scalars, 0, 64, stream));
+    CDH_CUDA(cudaMemsetAsync(out, 0, (size_t)n_hist * (size_t)n_bins * sizeof(uint64_t), stream));
+
+    int launches = 0;
+    // ---- K0 repack -----------------------------------------------------------------------------
+    if (frame_slots > 0) {
+        RepackParams rp;
+        rp.coords = (const float*)coords; rp.pk = ctx->d_pk;
+        rp.off = (const int32_t*)(d + b_segs + b_rows + b_boxes);
+        rp.pad_off = (const uint32_t*)(d + b_segs + b_rows + b_boxes + b_off);
+        rp.extent_bits = ctx->d_scalars + 1;
+        rp.boxes = (const BoxConst*)(d + b_segs + b_rows);
+        rp.n_species = n_species; rp.n_total = off[n_species]; rp.n_frames = n_frames;
+        rp.box_type = box_type; rp.n_boxes = nb > 0 ? nb : 1;
+        rp.frame_slots = frame_slots; rp.blocks_per_frame = (frame_slots + 255) / 256;
+        const uint64_t blocks = (uint64_t)rp.blocks_per_frame * (uint64_t)n_frames;
+        if (blocks > 0x7fffffffull) return CDH_ERR_INVALID_ARG;
+        repack_kernel<<<(unsigned)blocks, 256, 0, stream>>>(rp);
+        CDH_CUDA(cudaGetLastError());
+        ++launches;
+    }
+
+    // ---- K1 tile kernel(s) ---------------------------------------------------------------------
+    uint32_t grid = 0;
+    if (wt.n_items > 0) {
+        TileParams tp;
+        tp.pk = ctx->d_pk; tp.segs = (const Seg*)d; tp.rows = (const Row*)(d + b_segs);
+        tp.boxes = (const BoxConst*)(d + b_segs + b_rows);
+        tp.out = (unsigned long long*)out; tp.extent = (const float*)(ctx->d_scalars + 1);
+        tp.n_rows = (uint32_t)wt.rows.size() - 1; tp.n_items = (uint32_t)wt.n_items;
+        tp.n_bins = (uint32_t)n_bins; tp.tj = tj; tp.smem_bins = sp.bins_per_sweep;
+        tp.rmax = rmax_f; tp.scale = scale_f; tp.thr2_bits = d2_threshold_bits(rmax_f); tp.one = 1.0f;
+        // fast paths: |b^-1 dx| <= 2 * extent must stay <= 4 (triclinic pruning margin) / 2^21 (magic rint)
+        tp.extent_limit = use_simple_only ? -1.0f : (box_type == CDH_BOX_TRICLINIC ? 2.0f : 1048576.0f);
+        grid = grid_full < tp.n_items ? grid_full : tp.n_items;
+        const bool run_fast = !use_simple_only;
+        const bool run_simple = use_simple_only || box_type != CDH_BOX_NONE;
+        if (run_fast) {
+            tp.counter = ctx->d_scalars;
+            CDH_CUDA(cudaFuncSetAttribute((const void*)vf.fn, cudaFuncAttributeMaxDynamicSharedMemorySize, smem_bytes));
+            vf.fn<<<grid, vf.threads, smem_bytes, stream>>>(tp);
+            CDH_CUDA(cudaGetLastError());
+            ++launches;
+        }
+        if (run_simple) {
+            tp.counter = ctx->d_scalars + 2;
+            CDH_CUDA(cudaFuncSetAttribute((const void*)vs.fn, cudaFuncAttributeMaxDynamicSharedMemorySize, smem_bytes));
+            vs.fn<<<grid, vs.threads, smem_bytes, stream>>>(tp);
+            CDH_CUDA(cudaGetLastError());
+            ++launches;
+        }
+    }
+    ctx->info[0] = launches; ctx->info[1] = (int64_t)wt.n_items; ctx->info[2] = sp.n_sweeps; ctx->info[3] = grid;
+    ctx->info[4] = vf.threads; ctx->info[5] = smem_bytes;
+    ctx->info[6] = (use_simple_only ? 0 : 1) | (box_type << 4) | (tri << 8) | ((int)split << 12) | ((int)big << 13) | ((int64_t)tj << 16);
+    ctx->info[7] = (int64_t)wt.padded_pairs;
+    return CDH_OK;
+}
+
+extern "C" int cdh_histograms_host(cdh_ctx* ctx, const void* coords, int32_t n_frames, const int32_t* off,
+                                   int32_t n_species, int32_t box_type, const double* box, int32_t n_boxes,
+                                   double r_max, int32_t n_bins, int32_t precision, void* stream_, uint64_t* out) {
+    if (!ctx) return CDH_ERR_INVALID_ARG;
+    int rc = validate(coords, n_frames, off, n_species, box_type, box, n_boxes, r_max, n_bins, precision, out);
+    if (rc != CDH_OK) return rc;
+    cudaStream_t stream = (cudaStream_t)stream_;
+    DeviceGuard guard(ctx->device);
+    if (!guard.ok) return cuda_fail(ctx, cudaGetLastError(), "cudaSetDevice");
+    const size_t cbytes = (size_t)n_frames * (size_t)off[n_species] * 3 * sizeof(float);
+    const size_t obytes = (size_t)(n_species * (n_species + 1) / 2) * (size_t)n_bins * sizeof(uint64_t);
+    if ((rc = grow(ctx, &ctx->d_io_coords, &ctx->io_coords_bytes, cbytes > 0 ? cbytes : 16, false)) != CDH_OK) return rc;
+    if ((rc = grow(ctx, &ctx->d_io_out, &ctx->io_out_bytes, obytes, false)) != CDH_OK) return rc;
+    if (cbytes) CDH_CUDA(cudaMemcpyAsync(ctx->d_io_coords, coords, cbytes, cudaMemcpyHostToDevice, stream));   // one H2D copy
+    rc = cdh_histograms(ctx, ctx->d_io_coords, n_frames, off, n_species, box_type, box, n_boxes, r_max, n_bins,
+                        precision, stream_, (uint64_t*)ctx->d_io_out);
+    if (rc != CDH_OK) return rc;
+    CDH_CUDA(cudaMemcpyAsync(out, ctx->d_io_out, obytes, cudaMemcpyDeviceToHost, stream));                      // one D2H copy
+    CDH_CUDA(cudaStreamSynchronize(stream));
+    return CDH_OK;
+}

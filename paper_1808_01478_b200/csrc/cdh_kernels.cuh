@@ -1,0 +1,137 @@
+// cdh_kernels.cuh -- the CUDA kernels of libcdh (sm_100a).
+//
+//   K0 repack_kernel      S0: AoS xyz -> padded groups of 4 (cdh_device.cuh), coordinate extent
+//   K1 tile_kernel<...>   S1 tile schedule, S2 distance, S3 minimum image, S4 bin, S5 private
+//                         shared-memory histogram, S6/S7 flush into the uint64 result
+// (step names: SURVEY.md 8a; the paper's analogue is the shared-memory kernel).
+//
+// The per-pair arithmetic reproduces DESIGN.md "Pinned sequence" bit for bit.  VAR_SIMPLE spells it
+// with the CUDA library's IEEE intrinsics (__fsub_rn, __fmul_rn, __fadd_rn, __fsqrt_rn, rintf, floorf);
+// VAR_FAST computes the same integers with packed f32x2 arithmetic, a magic-number rint/floor, a
+// Newton-corrected MUFU.RSQ square root and a threshold on d2.
+#pragma once
+#include "cdh_device.cuh"
+
+namespace cdh {
+
+constexpr int VAR_SIMPLE = 0;
+constexpr int VAR_FAST = 1;
+
+constexpr int BOX_NONE = 0, BOX_ORTHO = 1, BOX_TRI = 2;
+
+// Triclinic zero structure (skipping a term whose matrix entry is exactly 0 in B and in B^-1 changes
+// at most the sign of a zero, never d2): 0 general 3x3, 1 upper triangular (a along x, b in the xy
+// plane), 2 upper triangular with B[0][1] == 0 as well (the rhombic dodecahedron of config 3).
+constexpr int TRI_GENERAL = 0, TRI_UPPER = 1, TRI_UPPER_B01 = 2;
+
+// ---------------------------------------------------------------------------------------------
+// K0: repack.  One thread per padded particle slot of one frame.
+// ---------------------------------------------------------------------------------------------
+struct RepackParams {
+    const float* coords;        // [n_frames][n_total][3]
+    float* pk;                  // [n_frames][frame_groups][12]
+    const int32_t* off;         // device, [n_species+1] particle offsets
+    const uint32_t* pad_off;    // device, [n_species+1] padded particle offsets (multiples of kPadParticles)
+    unsigned int* extent_bits;  // device scalar, atomicMax of the bits of max_k |(b^-1 x)_k| (fractional extent)
+    const BoxConst* boxes;      // box constants (periodic boxes), one or n_frames
+    int32_t n_species, n_total, n_frames;
+    int32_t box_type, n_boxes;
+    uint32_t frame_slots;       // padded particles per frame
+    uint32_t blocks_per_frame;
+};
+
+__global__ void __launch_bounds__(256) repack_kernel(const RepackParams P) {
+    const uint32_t f = blockIdx.x / P.blocks_per_frame;
+    const uint32_t slot = (blockIdx.x % P.blocks_per_frame) * blockDim.x + threadIdx.x;
+    float m = 0.0f;
+    if (slot < P.frame_slots) {
+        // species of this slot: largest s with pad_off[s] <= slot
+        int lo = 0, hi = P.n_species;
+        while (hi - lo > 1) {
+            const int mid = (lo + hi) >> 1;
+            if (__ldg(P.pad_off + mid) <= slot) lo = mid; else hi = mid;
+        }
+        const uint32_t k = slot - __ldg(P.pad_off + lo);
+        const int32_t n = __ldg(P.off + lo + 1) - __ldg(P.off + lo);
+        float x = __int_as_float(0x7fc00000), y = x, z = x;   // NaN padding
+        if (k < (uint32_t)n) {
+            const float* c = P.coords + ((size_t)f * P.n_total + (size_t)__ldg(P.off + lo) + k) * 3;
+            x = c[0]; y = c[1]; z = c[2];
+            // Fractional extent |b^-1 x| (approximate, only compared against a limit with a wide margin).
+            // NaN compares false: a NaN coordinate does not raise the extent; its pairs are dropped anyway.
+            if (P.box_type == BOX_ORTHO) {
+                const BoxConst* bc = P.boxes + (P.n_boxes == 1 ? 0 : f);
+                m = fmaxf(fmaxf(fabsf(x * bc->invL[0]), fabsf(y * bc->invL[1])), fabsf(z * bc->invL[2]));
+            } else if (P.box_type == BOX_TRI) {
+                const BoxConst* bc = P.boxes + (P.n_boxes == 1 ? 0 : f);
+#pragma unroll
+                for (int k = 0; k < 3; ++k)
+                    m = fmaxf(m, fabsf(bc->Binv[3 * k] * x + bc->Binv[3 * k + 1] * y + bc->Binv[3 * k + 2] * z));
+            }
+        }
+        float* g = P.pk + ((size_t)f * (P.frame_slots / kGroup) + slot / kGroup) * kGroupFloats + (slot % kGroup);
+        g[0] = x; g[4] = y; g[8] = z;
+    }
+    // warp max, one atomic per warp (non-negative floats order like their bit patterns)
+    for (int o = 16; o > 0; o >>= 1) m = fmaxf(m, __shfl_xor_sync(0xffffffffu, m, o));
+    if ((threadIdx.x & 31) == 0 && m > 0.0f) atomicMax(P.extent_bits, __float_as_uint(m));
+}
+
+// ---------------------------------------------------------------------------------------------
+// Box constants staged in shared memory (triclinic) / registers (orthorhombic)
+// ---------------------------------------------------------------------------------------------
+struct OrthoRegs { float L[3], invL[3]; };
+
+// The pinned sequence for ONE pair, spelled with IEEE intrinsics.  Returns d2.
+// bc: box constants (global or shared memory pointer); only read for periodic boxes.
+template <int BOX>
+__device__ __forceinline__ float pair_d2_simple(float xi, float yi, float zi, float xj, float yj, float zj,
+                                                const BoxConst* __restrict__ bc) {
+    float dx = __fsub_rn(xj, xi), dy = __fsub_rn(yj, yi), dz = __fsub_rn(zj, zi);
+    if constexpr (BOX == BOX_ORTHO) {
+        float t, n;
+        t = __fmul_rn(dx, bc->invL[0]); n = rintf(t); dx = __fsub_rn(dx, __fmul_rn(bc->L[0], n));
+        t = __fmul_rn(dy, bc->invL[1]); n = rintf(t); dy = __fsub_rn(dy, __fmul_rn(bc->L[1], n));
+        t = __fmul_rn(dz, bc->invL[2]); n = rintf(t); dz = __fsub_rn(dz, __fmul_rn(bc->L[2], n));
+    } else if constexpr (BOX == BOX_TRI) {
+        float n[3], e[3];
+        const float d[3] = {dx, dy, dz};
+#pragma unroll
+        for (int k = 0; k < 3; ++k) {
+            const float s = __fadd_rn(__fadd_rn(__fmul_rn(bc->Binv[3 * k + 0], dx), __fmul_rn(bc->Binv[3 * k + 1], dy)),
+                                      __fmul_rn(bc->Binv[3 * k + 2], dz));
+            n[k] = rintf(s);
+        }
+#pragma unroll
+        for (int r = 0; r < 3; ++r) {
+            const float sh = __fadd_rn(__fadd_rn(__fmul_rn(bc->B[3 * r + 0], n[0]), __fmul_rn(bc->B[3 * r + 1], n[1])),
+                                       __fmul_rn(bc->B[3 * r + 2], n[2]));
+            e[r] = __fsub_rn(d[r], sh);
+        }
+        float best = __int_as_float(0x7f800000);
+#pragma unroll 1
+        for (int m = 0; m < 27; ++m) {
+            const float cx = __fadd_rn(e[0], bc->S[m][0]), cy = __fadd_rn(e[1], bc->S[m][1]),
+                        cz = __fadd_rn(e[2], bc->S[m][2]);
+            const float c2 = __fadd_rn(__fadd_rn(__fmul_rn(cx, cx), __fmul_rn(cy, cy)), __fmul_rn(cz, cz));
+            if (c2 < best) best = c2;
+        }
+        return best;
+    }
+    return __fadd_rn(__fadd_rn(__fmul_rn(dx, dx), __fmul_rn(dy, dy)), __fmul_rn(dz, dz));
+}
+
+// Binning of one d2 by the pinned sequence (library sqrt / floor).  hist = shared address of slot 0,
+// the CTA owns bins [bin_lo, bin_lo + lim).
+__device__ __forceinline__ void bin_simple(float d2, float rmax, float scale, uint32_t n_bins,
+                                           uint32_t hist, uint32_t bin_lo, uint32_t lim) {
+    const float d = __fsqrt_rn(d2);
+    if (d < rmax) {                                       // drops d >= r_max and NaN
+        uint32_t b = (uint32_t)floorf(__fmul_rn(d, scale));
+        b = min(b, n_bins - 1u);                          // reading Q3
+        b -= bin_lo;
+        if (b < lim) hist_inc(hist + 4u * b);
+    }
+}
+
+}  // namespace cdh

@@ -1,0 +1,206 @@
+// cdh_tile.cuh -- K1: the persistent tile kernel (steps S1-S7 of SURVEY.md 8a).
+//
+// One CTA owns one private uint32 histogram in shared memory (histogram strategy 3, PAPER.md:117-123,
+// and the paper's shared-memory kernel) and pulls work items (i-tile, j-chunk) from a
+// global counter.  Items are ordered by (histogram row, bin sweep), so a CTA flushes into the uint64
+// result only when that key changes, when its increment budget nears 2^32 and at exit.
+// Each thread keeps R = 4 i-particles in registers; the j-chunk streams through two 6 KB shared-memory
+// stages filled by 1-D TMA bulk copies (cp.async.bulk + mbarrier); all lanes read the same j-group
+// (LDS.128 broadcast).  Intra-species segments only schedule j-chunks that reach above the diagonal
+// (triangular schedule, Fig. 1, 223-225); tiles on the diagonal take the masked path.
+#pragma once
+#include <type_traits>
+#include "cdh_fast.cuh"
+
+namespace cdh {
+
+constexpr int kR = 4;                       // i-particles per thread (one group)
+constexpr int kSmemHeader = 128;            // mbarriers + scheduler slot
+constexpr uint64_t kMaxIncrements = 0xFFFFFFFFull;
+
+__host__ __device__ constexpr int tile_smem_bytes(int smem_bins) {
+    return kSmemHeader + 2 * kStageBytes + sizeof(BoxConst) + 16 + 4 * (smem_bins + 1);
+}
+
+template <int BOX, int TRI, int T, int VAR, bool SPLIT, int MINB>
+__global__ void __launch_bounds__(T, MINB) tile_kernel(const TileParams P) {
+    extern __shared__ __align__(128) unsigned char smem[];
+    constexpr int TI = T * kR;
+    uint64_t* bars = reinterpret_cast<uint64_t*>(smem);
+    volatile uint32_t* s_item = reinterpret_cast<volatile uint32_t*>(smem + 16);
+    float* stage0 = reinterpret_cast<float*>(smem + kSmemHeader);
+    BoxConst* s_box = reinterpret_cast<BoxConst*>(smem + kSmemHeader + 2 * kStageBytes);
+    uint32_t* s_hist = reinterpret_cast<uint32_t*>(smem + kSmemHeader + 2 * kStageBytes + sizeof(BoxConst) + 16);
+    const uint32_t hist_addr = smem_u32(s_hist);
+    const uint32_t bar_addr = smem_u32(bars);
+    const uint32_t stage_addr = smem_u32(stage0);
+    const int tid = threadIdx.x;
+
+    // The fast variants are exact only while the coordinate extent keeps |b^-1 dx| small (magic-number
+    // rint, pruning margin); otherwise this launch does nothing and the VAR_SIMPLE launch that follows
+    // it does the work (and vice versa).  Uniform over the grid.
+    if constexpr (BOX != BOX_NONE) {
+        const bool fast_ok = __ldg(P.extent) <= P.extent_limit;
+        if ((VAR == VAR_FAST) != fast_ok) return;
+    }
+
+    if (tid == 0) { mbar_init(bar_addr, 1); mbar_init(bar_addr + 8, 1); fence_mbar_init(); }
+    for (uint32_t b = tid; b <= P.smem_bins; b += T) s_hist[b] = 0;
+    __syncthreads();
+
+    uint32_t stage_cnt = 0;                 // stages consumed so far: buffer = cnt & 1, parity = (cnt >> 1) & 1
+    uint32_t cur_key = 0xFFFFFFFFu, cur_hist = 0, cur_lo = 0, cur_lim = 0, cur_box = 0xFFFFFFFFu;
+    uint64_t increments = 0;                // upper bound of increments since the last flush
+    const f2 ONE = dup2(P.one);
+    const f2 SCALE = dup2(P.scale);
+
+    auto flush = [&]() {
+        __syncthreads();
+        if (cur_key != 0xFFFFFFFFu) {
+            unsigned long long* o = P.out + (size_t)cur_hist * P.n_bins;
+            for (uint32_t b = tid; b < cur_lim; b += T) {
+                const uint32_t v = s_hist[b];
+                if (v) {
+                    s_hist[b] = 0;
+                    atomicAdd(o + min(cur_lo + b, P.n_bins - 1u), (unsigned long long)v);   // Q3 slot -> last bin
+                }
+            }
+        }
+        increments = 0;
+        __syncthreads();
+    };
+
+    for (;;) {
+        if (tid == 0) *s_item = atomicAdd(P.counter, 1u);
+        __syncthreads();
+        const uint32_t item = *s_item;
+        if (item >= P.n_items) break;
+
+        // row of the item: largest r with rows[r].item_prefix <= item
+        uint32_t lo = 0, hi = P.n_rows;
+        while (hi - lo > 1) {
+            const uint32_t mid = (lo + hi) >> 1;
+            if (__ldg(&P.rows[mid].item_prefix) <= item) lo = mid; else hi = mid;
+        }
+        const Row row = P.rows[lo];
+        const Seg seg = P.segs[row.seg];
+        const uint32_t jc = row.jc0 + (item - row.item_prefix);
+        const uint32_t j0 = jc * P.tj;
+        const uint32_t j1 = min((uint32_t)seg.nj, j0 + P.tj);
+        const uint32_t i0 = row.i0;
+
+        if (seg.key != cur_key || increments + (uint64_t)TI * P.tj > kMaxIncrements) {
+            flush();
+            cur_key = seg.key; cur_hist = seg.hist; cur_lo = seg.bin_lo;
+            cur_lim = seg.bin_cnt + seg.last_sweep;
+        }
+        increments += (uint64_t)TI * P.tj;
+        if (BOX != BOX_NONE && seg.box != cur_box) {
+            __syncthreads();
+            const float* src = reinterpret_cast<const float*>(P.boxes + seg.box);
+            for (int k = tid; k < (int)(sizeof(BoxConst) / 4); k += T) reinterpret_cast<float*>(s_box)[k] = __ldg(src + k);
+            cur_box = seg.box;
+            __syncthreads();
+        }
+
+        // my R = 4 i-particles: one group
+        const float4* gi = reinterpret_cast<const float4*>(P.pk + ((size_t)seg.i_group + (i0 >> 2) + tid) * kGroupFloats);
+        const float4 XI = __ldg(gi), YI = __ldg(gi + 1), ZI = __ldg(gi + 2);
+        const float xi[4] = {XI.x, XI.y, XI.z, XI.w}, yi[4] = {YI.x, YI.y, YI.z, YI.w}, zi[4] = {ZI.x, ZI.y, ZI.z, ZI.w};
+        const uint32_t ig = i0 + 4u * tid;          // index of my first i-particle inside the species
+
+        const bool masked = seg.same && (j0 < i0 + TI);       // some j <= some i: test j > i per pair
+        const uint32_t n_stage = (j1 - j0 + kStageParticles - 1) / kStageParticles;
+        const uint32_t s_begin = (masked && i0 > j0) ? (i0 - j0) / kStageParticles : 0;   // stages wholly below the diagonal
+        const float* jsrc = P.pk + ((size_t)seg.j_group + (j0 >> 2)) * kGroupFloats;
+
+        FastBox fb;
+        if constexpr (VAR == VAR_FAST && BOX == BOX_ORTHO) {
+#pragma unroll
+            for (int k = 0; k < 3; ++k) { fb.L[k] = s_box->L[k]; fb.invL[k] = s_box->invL[k]; }
+        }
+        if constexpr (VAR == VAR_FAST && BOX == BOX_TRI) {
+#pragma unroll
+            for (int k = 0; k < 9; ++k) { fb.B[k] = s_box->B[k]; fb.Binv[k] = s_box->Binv[k]; }
+        }
+        const bool prune = (BOX == BOX_TRI) ? (s_box->prune_ok != 0.0f) : true;
+        const uint32_t addr_c = hist_addr - 4u * (kFloorMagicBits + cur_lo);
+        const uint32_t sub_c = kFloorMagicBits + cur_lo;
+
+        if (tid == 0 && s_begin < n_stage) {
+            const uint32_t b = stage_cnt & 1u;
+            mbar_expect_tx(bar_addr + 8 * b, kStageBytes);
+            tma_load_1d(stage_addr + b * kStageBytes, jsrc + (size_t)s_begin * kStageGroups * kGroupFloats, kStageBytes, bar_addr + 8 * b);
+        }
+        for (uint32_t s = s_begin; s < n_stage; ++s) {
+            const uint32_t b = stage_cnt & 1u;
+            if (tid == 0 && s + 1 < n_stage) {
+                const uint32_t nb = b ^ 1u;
+                mbar_expect_tx(bar_addr + 8 * nb, kStageBytes);
+                tma_load_1d(stage_addr + nb * kStageBytes, jsrc + (size_t)(s + 1) * kStageGroups * kGroupFloats, kStageBytes, bar_addr + 8 * nb);
+            }
+            mbar_wait(bar_addr + 8 * b, (stage_cnt >> 1) & 1u);
+            const float4* sj = reinterpret_cast<const float4*>(stage0 + b * (kStageBytes / 4));
+            const uint32_t jbase = j0 + s * kStageParticles;                   // species index of the stage's first j
+            const uint32_t n_grp = (min(j1 - jbase, (uint32_t)kStageParticles) + 3u) >> 2;
+
+            auto body = [&](auto masked_c) {
+                constexpr bool MASKED = decltype(masked_c)::value;
+#pragma unroll 1
+                for (uint32_t g = 0; g < n_grp; ++g) {
+                    const float4 XJ = sj[3 * g], YJ = sj[3 * g + 1], ZJ = sj[3 * g + 2];
+                    const uint32_t jg = jbase + 4u * g;
+                    if constexpr (VAR == VAR_SIMPLE) {
+                        const float xj[4] = {XJ.x, XJ.y, XJ.z, XJ.w}, yj[4] = {YJ.x, YJ.y, YJ.z, YJ.w}, zj[4] = {ZJ.x, ZJ.y, ZJ.z, ZJ.w};
+#pragma unroll
+                        for (int c = 0; c < 4; ++c)
+#pragma unroll
+                            for (int r = 0; r < kR; ++r) {
+                                if (MASKED && !(jg + c > ig + r)) continue;
+                                const float d2 = pair_d2_simple<BOX>(xi[r], yi[r], zi[r], xj[c], yj[c], zj[c], s_box);
+                                bin_simple(d2, P.rmax, P.scale, P.n_bins, hist_addr, cur_lo, cur_lim);
+                            }
+                    } else {
+                        const f2 XA = pk2(XJ.x, XJ.y), XB = pk2(XJ.z, XJ.w), YA = pk2(YJ.x, YJ.y), YB = pk2(YJ.z, YJ.w),
+                                 ZA = pk2(ZJ.x, ZJ.y), ZB = pk2(ZJ.z, ZJ.w);
+#pragma unroll
+                        for (int r = 0; r < kR; ++r) {
+#pragma unroll
+                            for (int hlf = 0; hlf < 2; ++hlf) {
+                                bool nf0, nf1;
+                                f2 d2 = pair_d2_fast<BOX, TRI>(hlf ? XB : XA, hlf ? YB : YA, hlf ? ZB : ZA, xi[r], yi[r], zi[r], fb, ONE, nf0, nf1);
+                                bool k0 = true, k1 = true;
+                                if constexpr (MASKED) { k0 = jg + 2 * hlf > ig + r; k1 = jg + 2 * hlf + 1 > ig + r; }
+                                if constexpr (BOX == BOX_TRI) {
+                                    // zero-shift candidate is decisive unless a fractional coordinate is within
+                                    // kPruneDelta of +-1/2 (or pruning is not allowed for this box / r_max)
+                                    nf0 = (nf0 || !prune) && k0; nf1 = (nf1 || !prune) && k1;
+                                    if (nf0 || nf1) {
+                                        const int c0 = 2 * hlf;
+                                        const float xa = c0 ? XJ.z : XJ.x, ya = c0 ? YJ.z : YJ.x, za = c0 ? ZJ.z : ZJ.x;
+                                        const float xb = c0 ? XJ.w : XJ.y, yb = c0 ? YJ.w : YJ.y, zb = c0 ? ZJ.w : ZJ.y;
+                                        float p, q; upk2(d2, p, q);
+                                        if (nf0) p = pair_d2_simple<BOX_TRI>(xi[r], yi[r], zi[r], xa, ya, za, s_box);
+                                        if (nf1) q = pair_d2_simple<BOX_TRI>(xi[r], yi[r], zi[r], xb, yb, zb, s_box);
+                                        d2 = pk2(p, q);
+                                    }
+                                }
+                                bin_fast2<SPLIT>(d2, k0, k1, SCALE, ONE, P.thr2_bits, addr_c, hist_addr, sub_c, cur_lim);
+                            }
+                        }
+                    }
+                }
+            };
+            // only stages that touch the diagonal band need the mask
+            const bool stage_masked = masked && (jbase < i0 + TI);
+            if (stage_masked) body(std::true_type{}); else body(std::false_type{});
+
+            __syncthreads();          // everyone is done with buffer b before it is refilled
+            ++stage_cnt;
+        }
+        __syncthreads();              // s_item is rewritten at the top of the loop
+    }
+    flush();
+}
+
+}  // namespace cdh
