@@ -53,6 +53,8 @@ extern "C" {
 #define CDH_FLAG_NO_PRUNE        (1u << 1) /* triclinic: always search the 27 shifts */
 #define CDH_FLAG_WARP_AGGREGATE  (1u << 2) /* always aggregate equal bins in a warp (__match_any_sync) */
 #define CDH_FLAG_NO_AGGREGATE    (1u << 3) /* never aggregate */
+#define CDH_FLAG_TIME_KERNELS     (1u << 4) /* record CUDA events around the tile kernel(s) of every call
+                                              (measurement; read with cdh_last_call_kernel_ms) */
 #define CDH_FLAG_MAX_SMEM_BINS_SHIFT 8     /* bits 8..31: if non-zero, cap on the bins one CTA keeps in
                                               shared memory (forces the bin-range-split path) */
 
@@ -121,6 +123,13 @@ const char *cdh_last_error(const cdh_ctx *ctx);
  *   info[6] = kernel variant id                  info[7] = evaluated pairs incl. padding lanes (low 32 bits unused; see info64)
  * Returns CDH_OK or CDH_ERR_INVALID_ARG. */
 int cdh_last_call_info(const cdh_ctx *ctx, int64_t info[8]);
+
+/* Device time of the LAST cdh_histograms call on a context created with CDH_FLAG_TIME_KERNELS, from CUDA
+ * events recorded on the call's stream:  ms[0] = the tile kernel launch(es) (steps S1-S7),
+ * ms[1] = the whole call (scratch upload, zeroing, repack, tile kernels).  WAITS for the call's last
+ * event (host blocks until the call's device work is done).  Returns CDH_OK, CDH_ERR_INVALID_ARG (no
+ * such flag / no call yet / NULL) or CDH_ERR_CUDA. */
+int cdh_last_call_kernel_ms(cdh_ctx *ctx, double ms[2]);
 
 #ifdef __cplusplus
 }

@@ -23,10 +23,11 @@ FLAG_SIMPLE_KERNEL = 1 << 0
 FLAG_NO_PRUNE = 1 << 1
 FLAG_WARP_AGGREGATE = 1 << 2
 FLAG_NO_AGGREGATE = 1 << 3
+FLAG_TIME_KERNELS = 1 << 4
 FLAG_MAX_SMEM_BINS_SHIFT = 8
 
 EXPORTS = ["cdh_create", "cdh_histograms", "cdh_histograms_host", "cdh_destroy", "cdh_strerror",
-           "cdh_last_error", "cdh_last_call_info",
+           "cdh_last_error", "cdh_last_call_info", "cdh_last_call_kernel_ms",
            "cdh_bench_fp32_rate", "cdh_bench_shared_atomics", "cdh_selftest_sqrt"]
 
 
@@ -65,6 +66,8 @@ def load(path: Optional[str] = None) -> ctypes.CDLL:
     lib.cdh_last_error.argtypes = [vp]
     lib.cdh_last_call_info.restype = ctypes.c_int
     lib.cdh_last_call_info.argtypes = [vp, ctypes.POINTER(ctypes.c_int64)]
+    lib.cdh_last_call_kernel_ms.restype = ctypes.c_int
+    lib.cdh_last_call_kernel_ms.argtypes = [vp, ctypes.POINTER(dbl)]
     lib.cdh_bench_fp32_rate.restype = ctypes.c_int
     lib.cdh_bench_fp32_rate.argtypes = [ctypes.c_int, ctypes.c_int, vp, ctypes.POINTER(dbl), ctypes.POINTER(dbl)]
     lib.cdh_bench_shared_atomics.restype = ctypes.c_int
@@ -168,6 +171,12 @@ class Context:
         return {"launches": v[0], "items": v[1], "sweeps": v[2], "ctas": v[3], "threads": v[4],
                 "smem_bytes": v[5], "variant": v[6], "tj": v[6] >> 16, "fast": bool(v[6] & 1),
                 "padded_pairs": v[7]}
+
+    def last_call_kernel_ms(self):
+        """(tile kernel ms, whole call ms) of the last call; needs FLAG_TIME_KERNELS; waits for the call."""
+        arr = (ctypes.c_double * 2)()
+        self._check(self._lib.cdh_last_call_kernel_ms(self._h, arr))
+        return float(arr[0]), float(arr[1])
 
     def cdh_destroy(self) -> None:
         if self._h:

@@ -1,0 +1,244 @@
+"""-m gpu: parity of the CUDA path (through the C ABI, include/cdh.h) with the CPU oracle, bin for bin.
+
+Bar (BASELINE.json north_star): uint64 histograms BIT-EXACT to the fp32 oracle.  Every kernel variant
+(production packed-f32x2 kernel, the plain cross-validation kernel, the bin-range-split path, forced
+27-shift triclinic search) must give the same integers ("cross validation").
+"""
+import hashlib
+import math
+
+import numpy as np
+import pytest
+
+import paper_1808_01478_b200 as cdh
+from paper_1808_01478_b200 import inputs
+from oracle import oracle as cdh_oracle
+
+torch = pytest.importorskip("torch")
+pytestmark = pytest.mark.gpu
+
+
+def _need_gpu():
+    if not torch.cuda.is_available():
+        pytest.skip("no CUDA device")
+
+
+def gpu_hist(p, flags=0, host=False):
+    _need_gpu()
+    with cdh.Context(0, flags) as ctx:
+        if host:
+            return ctx.cdh_histograms_host(p.coords, p.species_offsets, p.box_type, p.box, p.r_max, p.n_bins), \
+                ctx.last_call_info()
+        out = cdh.histograms_device(ctx, p)
+        torch.cuda.synchronize()
+        return out.cpu().numpy().view(np.uint64), ctx.last_call_info()
+
+
+def assert_same(got, want, what):
+    if not np.array_equal(got, want):
+        diff = got.astype(np.int64) - want.astype(np.int64)
+        rows, bins = np.nonzero(diff)
+        raise AssertionError(f"{what}: {len(rows)} bins differ, L1={int(np.abs(diff).sum())}, "
+                             f"sum got={int(got.sum())} want={int(want.sum())}, first at row {rows[0]} bin {bins[0]}: "
+                             f"{int(got[rows[0], bins[0]])} vs {int(want[rows[0], bins[0]])}")
+
+
+_oracle_cache = {}
+
+
+def oracle_hist(p):
+    key = (hashlib.sha1(p.coords.tobytes()).hexdigest(), tuple(p.species_offsets.tolist()), p.n_bins, p.r_max,
+           p.box_type, None if p.box is None else p.box.tobytes())
+    if key not in _oracle_cache:
+        _oracle_cache[key] = cdh_oracle.problem_histograms(p, "f32")
+    return _oracle_cache[key]
+
+
+FLAG_SETS = {
+    "fast": 0,
+    "simple": cdh.FLAG_SIMPLE_KERNEL,
+    "split3000": 3000 << cdh.FLAG_MAX_SMEM_BINS_SHIFT,
+    "simple_split700": cdh.FLAG_SIMPLE_KERNEL | (700 << cdh.FLAG_MAX_SMEM_BINS_SHIFT),
+}
+
+
+@pytest.mark.parametrize("variant", sorted(FLAG_SETS))
+@pytest.mark.parametrize("k", [1, 2, 3, 4, 5])
+def test_reduced_configs_bit_exact(k, variant):
+    p = inputs.reduced_config(k)
+    got, info = gpu_hist(p, FLAG_SETS[variant])
+    assert_same(got, oracle_hist(p), f"{p.name} [{variant}] {info}")
+    cap = FLAG_SETS[variant] >> cdh.FLAG_MAX_SMEM_BINS_SHIFT
+    if cap and p.n_bins > cap:
+        assert info["sweeps"] == -(-p.n_bins // cap)
+
+
+def test_config1_full_and_total_count():
+    p = inputs.config1()
+    got, _ = gpu_hist(p)
+    assert int(got.sum()) == 1_999_000          # P1: N(N-1)/2, r_max covers all pairs
+    assert_same(got, oracle_hist(p), p.name)
+
+
+def test_host_entry_point_matches_device_entry_point():
+    p = inputs.reduced_config(2)
+    a, _ = gpu_hist(p)
+    b, _ = gpu_hist(p, host=True)
+    assert_same(b, a, "cdh_histograms_host vs cdh_histograms")
+    assert_same(b, oracle_hist(p), "cdh_histograms_host")
+
+
+def test_triclinic_no_prune_equals_prune_and_oracle():
+    p = inputs.reduced_config(3)
+    a, _ = gpu_hist(p)
+    b, _ = gpu_hist(p, cdh.FLAG_NO_PRUNE)
+    assert_same(b, a, "27-shift search vs exact pruning")
+    assert_same(a, oracle_hist(p), p.name)
+
+
+def test_triclinic_beyond_half_height_runs_full_search():
+    # r_max > h_min/2: Eq. 5 alone is not exact; the neighbour search decides.
+    p = inputs.config3(counts=(1500, 2100), n_bins=4000, r_max=6.0)
+    got, _ = gpu_hist(p)
+    assert_same(got, oracle_hist(p), "cfg3 r_max=6")
+
+
+def test_triclinic_general_box_and_far_outside_coordinates():
+    box = np.array([[9.0, 0.5, -0.25], [1.5, 8.0, 0.75], [-2.0, 2.5, 7.0]])
+    heights_min = 5.0
+    for spread, tag in ((1.0, "inside"), (3.5, "outside")):
+        p = inputs.uniform_problem(77, (900, 1300), inputs.BOX_TRICLINIC, 3000, heights_min / 2, box=box, spread=spread)
+        got, info = gpu_hist(p)
+        assert_same(got, oracle_hist(p), f"general triclinic {tag} {info}")
+
+
+def test_upper_triangular_box_variant():
+    box = np.array([[10.0, 0.0, 0.0], [3.0, 9.0, 0.0], [-2.0, 4.0, 8.0]])
+    p = inputs.uniform_problem(78, (1000, 1200), inputs.BOX_TRICLINIC, 2500, 3.9, box=box)
+    got, info = gpu_hist(p)
+    assert_same(got, oracle_hist(p), f"upper triangular {info}")
+
+
+def test_ortho_unwrapped_coordinates_and_per_frame_boxes():
+    g = np.random.Generator(np.random.PCG64(5))
+    n, f = 2100, 3
+    coords = (g.random((f, n, 3)) * 30.0 - 10.0).astype(np.float32)      # several box lengths outside
+    boxes = np.stack([np.diag([6.0 + k, 7.0, 8.0 - k]) for k in range(f)]).reshape(f, 9)
+    p = inputs.Problem("ortho_per_frame_boxes", coords, np.array([0, 600, n], dtype=np.int32), inputs.BOX_ORTHO,
+                       boxes, 2.9, 1234)
+    got, _ = gpu_hist(p)
+    assert_same(got, oracle_hist(p), p.name)
+
+
+def test_p2_hand_example_species_split():
+    pts = np.array([[0, 0, 0], [3, 4, 0], [3, 4, 12], [0, 0, 12]], dtype=np.float32)[None]
+    p = inputs.Problem("p2", pts, np.array([0, 2, 4], dtype=np.int32), inputs.BOX_NONE, None, 16.0, 16)
+    got, _ = gpu_hist(p)
+    want = np.zeros((3, 16), dtype=np.uint64)
+    want[0, 5] = 1; want[1, 12] = 2; want[1, 13] = 2; want[2, 5] = 1          # SURVEY.md 8c pin P2
+    assert_same(got, want, "P2 hand example")
+    p13 = inputs.Problem("p2b", pts, np.array([0, 4], dtype=np.int32), inputs.BOX_NONE, None, 13.0, 13)
+    got, _ = gpu_hist(p13)
+    want = np.zeros((1, 13), dtype=np.uint64); want[0, 5] = 2; want[0, 12] = 2   # d = 13 dropped (Q2)
+    assert_same(got, want, "P2 r_max=13")
+
+
+def test_p4_triclinic_hand_example():
+    pts = np.array([[1, 1, 1], [8, 8, 2], [2, 14, 9], [13, 3, 15]], dtype=np.float32)[None]
+    box = np.array([[16.0, 0, 0], [0, 16.0, 0], [8.0, 8.0, 16.0]]).reshape(1, 9)
+    p = inputs.Problem("p4", pts, np.array([0, 4], dtype=np.int32), inputs.BOX_TRICLINIC, box, 16.0, 16)
+    got, _ = gpu_hist(p)
+    want = np.zeros((1, 16), dtype=np.uint64); want[0, 5] = 1; want[0, 7] = 1; want[0, 8] = 1; want[0, 9] = 3
+    assert_same(got, want, "P4 hand example")
+
+
+def test_p8_single_bin_exceeds_uint32():
+    # 100,000 identical points: bin 0 = 4,999,950,000 > 2^32 (flush rule)
+    pts = np.full((1, 100_000, 3), 0.25, dtype=np.float32)
+    p = inputs.Problem("p8", pts, np.array([0, 100_000], dtype=np.int32), inputs.BOX_NONE, None, 1.0, 64)
+    got, _ = gpu_hist(p)
+    assert int(got[0, 0]) == 4_999_950_000 and int(got.sum()) == 4_999_950_000
+
+
+def test_p9_wide_bin_split():
+    p = inputs.uniform_problem(9, (6000,), inputs.BOX_NONE, 1_000_000, math.sqrt(3.0))
+    got, info = gpu_hist(p)
+    assert info["sweeps"] > 1
+    assert_same(got, oracle_hist(p), f"1M bins {info}")
+
+
+def test_empty_species_tiny_inputs_and_nan():
+    pts = np.array([[0.1, 0.2, 0.3], [0.5, 0.5, 0.5], [np.nan, 0.0, 0.0], [0.9, 0.1, 0.4]], dtype=np.float32)[None]
+    p = inputs.Problem("tiny", pts, np.array([0, 0, 1, 1, 4], dtype=np.int32), inputs.BOX_NONE, None, 2.0, 7)
+    got, _ = gpu_hist(p)
+    assert_same(got, oracle_hist(p), "empty species + NaN")
+    one = inputs.Problem("one", pts[:, :1], np.array([0, 1], dtype=np.int32), inputs.BOX_NONE, None, 2.0, 7)
+    got, _ = gpu_hist(one)
+    assert int(got.sum()) == 0
+
+
+def test_q3_clamp_and_rmax_cut():
+    # distances at and just below r_max; scale rounding can push d*scale to n_bins (Q3)
+    r = np.float32(0.7)
+    xs = [np.nextafter(r, np.float32(0)), r, np.nextafter(r, np.float32(1)), np.float32(0.35), np.float32(0.0)]
+    pts = np.zeros((1, 1 + len(xs), 3), dtype=np.float32)
+    pts[0, 1:, 0] = xs
+    for n_bins in (1, 3, 7, 1000, 4097):
+        p = inputs.Problem(f"q3_{n_bins}", pts, np.array([0, 1, 1 + len(xs)], dtype=np.int32), inputs.BOX_NONE, None,
+                           float(r), n_bins)
+        got, _ = gpu_hist(p)
+        assert_same(got, oracle_hist(p), p.name)
+
+
+def test_sqrt_selftest_sample():
+    _need_gpu()
+    # full range is bench.py --selftest; here 2^26 patterns around 1.0 and the low end of the range
+    assert cdh.cdh_selftest_sqrt(0x3F000000, 0x3F000000 + (1 << 26)) == 0
+    assert cdh.cdh_selftest_sqrt(0x0D000000, 0x0D000000 + (1 << 24)) == 0
+
+
+def test_argument_errors_leave_out_untouched():
+    _need_gpu()
+    p = inputs.reduced_config(1)
+    dev = torch.device("cuda", 0)
+    coords = torch.from_numpy(p.coords).to(dev)
+    out = torch.full((1, p.n_bins), -7, dtype=torch.int64, device=dev)
+    with cdh.Context(0) as ctx:
+        for kw in (dict(n_bins=0), dict(r_max=-1.0), dict(r_max=float("nan")), dict(n_bins=(1 << 22) + 1)):
+            args = dict(r_max=p.r_max, n_bins=p.n_bins)
+            args.update(kw)
+            with pytest.raises(cdh.CdhError) as e:
+                ctx.cdh_histograms(coords, 1, p.species_offsets, p.box_type, None, args["r_max"], args["n_bins"], out)
+            assert e.value.code == cdh.binding.ERR_INVALID_ARG
+        with pytest.raises(cdh.CdhError) as e:
+            ctx.cdh_histograms(coords, 1, p.species_offsets, p.box_type, None, p.r_max, p.n_bins, out, precision=cdh.F64)
+        assert e.value.code == cdh.binding.ERR_UNSUPPORTED
+        with pytest.raises(cdh.CdhError):       # singular box
+            ctx.cdh_histograms(coords, 1, p.species_offsets, inputs.BOX_TRICLINIC, np.zeros((1, 9)), 1.0, 10, out)
+        with pytest.raises(cdh.CdhError):       # off-diagonal with ORTHO
+            ctx.cdh_histograms(coords, 1, p.species_offsets, inputs.BOX_ORTHO,
+                               np.array([[1.0, 0.1, 0, 0, 1, 0, 0, 0, 1]]), 1.0, 10, out)
+    torch.cuda.synchronize()
+    assert bool((out == -7).all())
+
+
+def test_context_reuse_growing_and_shrinking_problems():
+    _need_gpu()
+    with cdh.Context(0) as ctx:
+        for k in (1, 3, 2, 1, 5, 4):
+            p = inputs.reduced_config(k)
+            out = cdh.histograms_device(ctx, p)
+            torch.cuda.synchronize()
+            assert_same(out.cpu().numpy().view(np.uint64), oracle_hist(p), f"reuse {p.name}")
+
+
+def test_user_stream_and_back_to_back_calls():
+    _need_gpu()
+    p = inputs.reduced_config(2)
+    s = torch.cuda.Stream()
+    with cdh.Context(0) as ctx:
+        with torch.cuda.stream(s):
+            outs = [cdh.histograms_device(ctx, p, stream=s) for _ in range(3)]
+        s.synchronize()
+        for o in outs:
+            assert_same(o.cpu().numpy().view(np.uint64), oracle_hist(p), "stream")

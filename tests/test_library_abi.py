@@ -1,0 +1,73 @@
+"""-m "not gpu": libcdh.so builds, loads without a GPU and exports every symbol include/*.h declares;
+host-side argument validation returns error codes (no compute calls here)."""
+import ctypes
+import os
+import re
+
+import numpy as np
+import pytest
+
+from paper_1808_01478_b200 import binding
+from paper_1808_01478_b200 import build as cdh_build
+
+ROOT = os.path.dirname(os.path.dirname(os.path.abspath(__file__)))
+
+
+def declared_symbols():
+    names = set()
+    for h in ("cdh.h", "cdh_bench.h"):
+        text = open(os.path.join(ROOT, "include", h)).read()
+        text = re.sub(r"/\*.*?\*/", "", text, flags=re.S)
+        names.update(re.findall(r"\b(cdh_[a-z0-9_]+)\s*\(", text))
+    return sorted(names)
+
+
+@pytest.fixture(scope="module")
+def lib():
+    cdh_build.build()
+    return binding.load()
+
+
+def test_headers_declare_the_boundary():
+    names = declared_symbols()
+    for required in ("cdh_create", "cdh_histograms", "cdh_destroy"):
+        assert required in names
+    assert sorted(binding.EXPORTS) == names
+
+
+def test_library_exports_every_declared_symbol(lib):
+    for name in declared_symbols():
+        assert getattr(lib, name) is not None
+
+
+def test_strerror_texts(lib):
+    assert binding.cdh_strerror(0) == "ok"
+    assert "invalid" in binding.cdh_strerror(binding.ERR_INVALID_ARG)
+    assert "unsupported" in binding.cdh_strerror(binding.ERR_UNSUPPORTED)
+    assert "unknown" in binding.cdh_strerror(-99)
+
+
+def test_null_arguments_are_rejected_without_a_device(lib):
+    assert lib.cdh_create(None, 0, 0) == binding.ERR_INVALID_ARG
+    off = np.array([0, 4], dtype=np.int32)
+    rc = lib.cdh_histograms(None, 1, 1, off.ctypes.data, 1, 0, None, 0, 1.0, 8, 0, None, 1)
+    assert rc == binding.ERR_INVALID_ARG
+    assert lib.cdh_destroy(None) == binding.OK
+    info = (ctypes.c_int64 * 8)()
+    assert lib.cdh_last_call_info(None, info) == binding.ERR_INVALID_ARG
+
+
+def test_no_cpu_fallback_when_library_is_missing(tmp_path):
+    with pytest.raises(OSError):
+        binding.load(str(tmp_path / "libcdh_missing.so"))
+
+
+def test_product_does_not_import_the_oracle():
+    pkg = os.path.join(ROOT, "paper_1808_01478_b200")
+    for dirpath, _, files in os.walk(pkg):
+        for f in files:
+            if f.endswith((".py", ".cu", ".cuh", ".h")):
+                text = open(os.path.join(dirpath, f)).read()
+                assert not re.search(r"^\s*(from|import)\s+oracle\b", text, flags=re.M), f
+                assert not re.search(r"#include\s+[\"<][^\">]*oracle", text), f
+                assert "libcdh_oracle" not in text, f
