@@ -124,12 +124,15 @@ const char *cdh_last_error(const cdh_ctx *ctx);
  * Returns CDH_OK or CDH_ERR_INVALID_ARG. */
 int cdh_last_call_info(const cdh_ctx *ctx, int64_t info[8]);
 
-/* Device time of the LAST cdh_histograms call on a context created with CDH_FLAG_TIME_KERNELS, from CUDA
- * events recorded on the call's stream:  ms[0] = the tile kernel launch(es) (steps S1-S7),
- * ms[1] = the whole call (scratch upload, zeroing, repack, tile kernels).  WAITS for the call's last
- * event (host blocks until the call's device work is done).  Returns CDH_OK, CDH_ERR_INVALID_ARG (no
- * such flag / no call yet / NULL) or CDH_ERR_CUDA. */
-int cdh_last_call_kernel_ms(cdh_ctx *ctx, double ms[2]);
+/* Device time of a recent cdh_histograms call on a context created with CDH_FLAG_TIME_KERNELS, from CUDA
+ * events recorded on the call's stream (a ring of CDH_TIMED_CALLS event sets, one per call):
+ *   calls_back = 0 is the last call, 1 the one before, ... (< CDH_TIMED_CALLS and < calls made);
+ *   ms[0] = the tile kernel launch(es) (steps S1-S7),
+ *   ms[1] = the whole call (scratch upload, zeroing, repack, tile kernels).
+ * WAITS for that call's last event.  Returns CDH_OK, CDH_ERR_INVALID_ARG (no such flag / no such call /
+ * NULL) or CDH_ERR_CUDA. */
+#define CDH_TIMED_CALLS 256
+int cdh_call_kernel_ms(cdh_ctx *ctx, int calls_back, double ms[2]);
 
 #ifdef __cplusplus
 }

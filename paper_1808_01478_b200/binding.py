@@ -27,7 +27,7 @@ FLAG_TIME_KERNELS = 1 << 4
 FLAG_MAX_SMEM_BINS_SHIFT = 8
 
 EXPORTS = ["cdh_create", "cdh_histograms", "cdh_histograms_host", "cdh_destroy", "cdh_strerror",
-           "cdh_last_error", "cdh_last_call_info", "cdh_last_call_kernel_ms",
+           "cdh_last_error", "cdh_last_call_info", "cdh_call_kernel_ms",
            "cdh_bench_fp32_rate", "cdh_bench_shared_atomics", "cdh_selftest_sqrt"]
 
 
@@ -66,8 +66,8 @@ def load(path: Optional[str] = None) -> ctypes.CDLL:
     lib.cdh_last_error.argtypes = [vp]
     lib.cdh_last_call_info.restype = ctypes.c_int
     lib.cdh_last_call_info.argtypes = [vp, ctypes.POINTER(ctypes.c_int64)]
-    lib.cdh_last_call_kernel_ms.restype = ctypes.c_int
-    lib.cdh_last_call_kernel_ms.argtypes = [vp, ctypes.POINTER(dbl)]
+    lib.cdh_call_kernel_ms.restype = ctypes.c_int
+    lib.cdh_call_kernel_ms.argtypes = [vp, ctypes.c_int, ctypes.POINTER(dbl)]
     lib.cdh_bench_fp32_rate.restype = ctypes.c_int
     lib.cdh_bench_fp32_rate.argtypes = [ctypes.c_int, ctypes.c_int, vp, ctypes.POINTER(dbl), ctypes.POINTER(dbl)]
     lib.cdh_bench_shared_atomics.restype = ctypes.c_int
@@ -172,10 +172,10 @@ class Context:
                 "smem_bytes": v[5], "variant": v[6], "tj": v[6] >> 16, "fast": bool(v[6] & 1),
                 "padded_pairs": v[7]}
 
-    def last_call_kernel_ms(self):
-        """(tile kernel ms, whole call ms) of the last call; needs FLAG_TIME_KERNELS; waits for the call."""
+    def call_kernel_ms(self, calls_back: int = 0):
+        """(tile kernel ms, whole call ms) of a recent call (0 = last); needs FLAG_TIME_KERNELS; waits for it."""
         arr = (ctypes.c_double * 2)()
-        self._check(self._lib.cdh_last_call_kernel_ms(self._h, arr))
+        self._check(self._lib.cdh_call_kernel_ms(self._h, int(calls_back), arr))
         return float(arr[0]), float(arr[1])
 
     def cdh_destroy(self) -> None:

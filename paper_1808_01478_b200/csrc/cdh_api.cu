@@ -22,8 +22,8 @@ struct cdh_ctx {
     bool staged_pending = false;
     void* d_io_coords = nullptr; size_t io_coords_bytes = 0;  // cdh_histograms_host staging
     void* d_io_out = nullptr;    size_t io_out_bytes = 0;
-    cudaEvent_t ev[4] = {nullptr, nullptr, nullptr, nullptr};  // CDH_FLAG_TIME_KERNELS: call begin, tile begin, tile end, call end
-    bool timed = false;
+    cudaEvent_t* ev = nullptr;   // CDH_FLAG_TIME_KERNELS: ring of [CDH_TIMED_CALLS][4]: call begin, tile begin, tile end, call end
+    uint64_t timed_calls = 0;
     std::string err;
     int64_t info[8] = {0, 0, 0, 0, 0, 0, 0, 0};
 };
@@ -127,20 +127,26 @@ extern "C" int cdh_create(cdh_ctx** out, int device, uint32_t flags) {
         delete ctx;
         return CDH_ERR_ALLOC;
     }
-    if (flags & CDH_FLAG_TIME_KERNELS)
-        for (int k = 0; k < 4; ++k)
+    if (flags & CDH_FLAG_TIME_KERNELS) {
+        ctx->ev = new (std::nothrow) cudaEvent_t[4 * CDH_TIMED_CALLS]();
+        if (!ctx->ev) { cdh_destroy(ctx); return CDH_ERR_ALLOC; }
+        for (int k = 0; k < 4 * CDH_TIMED_CALLS; ++k)
             if (cudaEventCreate(&ctx->ev[k]) != cudaSuccess) { cudaGetLastError(); cdh_destroy(ctx); return CDH_ERR_ALLOC; }
+    }
     *out = ctx;
     return CDH_OK;
 }
 
-extern "C" int cdh_last_call_kernel_ms(cdh_ctx* ctx, double ms[2]) {
-    if (!ctx || !ms || !(ctx->flags & CDH_FLAG_TIME_KERNELS) || !ctx->timed) return CDH_ERR_INVALID_ARG;
+extern "C" int cdh_call_kernel_ms(cdh_ctx* ctx, int calls_back, double ms[2]) {
+    if (!ctx || !ms || !ctx->ev || calls_back < 0 || calls_back >= CDH_TIMED_CALLS ||
+        (uint64_t)calls_back >= ctx->timed_calls)
+        return CDH_ERR_INVALID_ARG;
     DeviceGuard g(ctx->device);
+    const cudaEvent_t* ev = ctx->ev + 4 * ((ctx->timed_calls - 1 - (uint64_t)calls_back) % CDH_TIMED_CALLS);
     float a = 0.f, b = 0.f;
-    CDH_CUDA(cudaEventSynchronize(ctx->ev[3]));
-    CDH_CUDA(cudaEventElapsedTime(&a, ctx->ev[1], ctx->ev[2]));
-    CDH_CUDA(cudaEventElapsedTime(&b, ctx->ev[0], ctx->ev[3]));
+    CDH_CUDA(cudaEventSynchronize(ev[3]));
+    CDH_CUDA(cudaEventElapsedTime(&a, ev[1], ev[2]));
+    CDH_CUDA(cudaEventElapsedTime(&b, ev[0], ev[3]));
     ms[0] = a; ms[1] = b;
     return CDH_OK;
 }
@@ -156,7 +162,10 @@ extern "C" int cdh_destroy(cdh_ctx* ctx) {
     if (ctx->d_io_coords) cudaFree(ctx->d_io_coords);
     if (ctx->d_io_out) cudaFree(ctx->d_io_out);
     if (ctx->staged) cudaEventDestroy(ctx->staged);
-    for (int k = 0; k < 4; ++k) if (ctx->ev[k]) cudaEventDestroy(ctx->ev[k]);
+    if (ctx->ev) {
+        for (int k = 0; k < 4 * CDH_TIMED_CALLS; ++k) if (ctx->ev[k]) cudaEventDestroy(ctx->ev[k]);
+        delete[] ctx->ev;
+    }
     cudaGetLastError();
     delete ctx;
     return CDH_OK;
@@ -260,8 +269,9 @@ extern "C" int cdh_histograms(cdh_ctx* ctx, const void* coords, int32_t n_frames
     std::memcpy(h + b_segs + b_rows + b_boxes, off, ((size_t)n_species + 1) * 4);
     std::memcpy(h + b_segs + b_rows + b_boxes + b_off, pad_off.data(), ((size_t)n_species + 1) * 4);
     char* d = (char*)ctx->d_tables;
-    const bool timing = (ctx->flags & CDH_FLAG_TIME_KERNELS) != 0;
-    if (timing) CDH_CUDA(cudaEventRecord(ctx->ev[0], stream));
+    const bool timing = ctx->ev != nullptr;
+    cudaEvent_t* ev = timing ? ctx->ev + 4 * (ctx->timed_calls % CDH_TIMED_CALLS) : nullptr;
+    if (timing) CDH_CUDA(cudaEventRecord(ev[0], stream));
     CDH_CUDA(cudaMemcpyAsync(d, h, tables, cudaMemcpyHostToDevice, stream));
     CDH_CUDA(cudaEventRecord(ctx->staged, stream));
     ctx->staged_pending = true;
@@ -289,7 +299,7 @@ extern "C" int cdh_histograms(cdh_ctx* ctx, const void* coords, int32_t n_frames
 
     // ---- K1 tile kernel(s) ---------------------------------------------------------------------
     uint32_t grid = 0;
-    if (timing) CDH_CUDA(cudaEventRecord(ctx->ev[1], stream));
+    if (timing) CDH_CUDA(cudaEventRecord(ev[1], stream));
     if (wt.n_items > 0) {
         TileParams tp;
         tp.pk = ctx->d_pk; tp.segs = (const Seg*)d; tp.rows = (const Row*)(d + b_segs);
@@ -319,9 +329,9 @@ extern "C" int cdh_histograms(cdh_ctx* ctx, const void* coords, int32_t n_frames
         }
     }
     if (timing) {
-        CDH_CUDA(cudaEventRecord(ctx->ev[2], stream));
-        CDH_CUDA(cudaEventRecord(ctx->ev[3], stream));
-        ctx->timed = true;
+        CDH_CUDA(cudaEventRecord(ev[2], stream));
+        CDH_CUDA(cudaEventRecord(ev[3], stream));
+        ++ctx->timed_calls;
     }
     ctx->info[0] = launches; ctx->info[1] = (int64_t)wt.n_items; ctx->info[2] = sp.n_sweeps; ctx->info[3] = grid;
     ctx->info[4] = vf.threads; ctx->info[5] = smem_bytes;
