@@ -34,17 +34,18 @@ def is_stale() -> bool:
     return any(os.path.getmtime(os.path.join(CSRC, d)) > t for d in DEPS)
 
 
-def build(force: bool = False, verbose: bool = False) -> str:
-    """Compile if the library is missing or older than a source; returns its path."""
-    if force or is_stale():
-        tmp = LIB + f".tmp{os.getpid()}"
-        cmd = [nvcc_path(), *NVCC_FLAGS, "-o", tmp, *[os.path.join(CSRC, s) for s in SOURCES]]
+def build(force: bool = False, verbose: bool = False, extra_flags=(), out: str = LIB) -> str:
+    """Compile if the library is missing or older than a source; returns its path.  ``extra_flags`` / ``out``
+    build an experimental copy (e.g. ``-DCDH_MINB=3``) next to the product library."""
+    if force or out != LIB or is_stale():
+        tmp = out + f".tmp{os.getpid()}"
+        cmd = [nvcc_path(), *NVCC_FLAGS, *extra_flags, "-o", tmp, *[os.path.join(CSRC, s) for s in SOURCES]]
         if verbose:
             cmd.insert(1, "-Xptxas=-v")
             print(" ".join(cmd), file=sys.stderr)
         subprocess.run(cmd, check=True, cwd=CSRC)
-        os.replace(tmp, LIB)
-    return LIB
+        os.replace(tmp, out)
+    return out
 
 
 if __name__ == "__main__":

@@ -63,10 +63,13 @@ int grow(cdh_ctx* ctx, void** p, size_t* have, size_t need, bool pinned_host) {
 typedef void (*TileFn)(const TileParams);
 struct Variant { TileFn fn; int threads; };
 
+#ifndef CDH_MINB
+#define CDH_MINB 2      // resident CTAs per SM the 256-thread fast variants are register-bounded for
+#endif
 template <int BOX, int TRI, bool SPLIT>
 Variant fast_variant(bool big) {
     if (big) return {tile_kernel<BOX, TRI, 512, VAR_FAST, SPLIT, 1>, 512};
-    return {tile_kernel<BOX, TRI, 256, VAR_FAST, SPLIT, 2>, 256};
+    return {tile_kernel<BOX, TRI, 256, VAR_FAST, SPLIT, CDH_MINB>, 256};
 }
 template <bool SPLIT>
 Variant pick_fast(int box_type, int tri, bool big) {
@@ -242,7 +245,11 @@ extern "C" int cdh_histograms(cdh_ctx* ctx, const void* coords, int32_t n_frames
     const Variant vf = split ? pick_fast<true>(box_type, tri, big) : pick_fast<false>(box_type, tri, big);
     const Variant vs = pick_simple(box_type, big);
     const uint32_t ti = (uint32_t)vf.threads * kR;
-    const uint32_t grid_full = (uint32_t)ctx->n_sm * (big ? 1u : 2u);
+    CDH_CUDA(cudaFuncSetAttribute((const void*)vf.fn, cudaFuncAttributeMaxDynamicSharedMemorySize, smem_bytes));
+    int resident = 0;      // CTAs of the production variant that fit one SM (registers, shared memory)
+    CDH_CUDA(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&resident, (const void*)vf.fn, vf.threads, (size_t)smem_bytes));
+    if (resident < 1) resident = 1;
+    const uint32_t grid_full = (uint32_t)ctx->n_sm * (uint32_t)resident;
 
     WorkTables wt;
     uint32_t tj = 8192;
@@ -315,7 +322,6 @@ extern "C" int cdh_histograms(cdh_ctx* ctx, const void* coords, int32_t n_frames
         const bool run_simple = use_simple_only || box_type != CDH_BOX_NONE;
         if (run_fast) {
             tp.counter = ctx->d_scalars;
-            CDH_CUDA(cudaFuncSetAttribute((const void*)vf.fn, cudaFuncAttributeMaxDynamicSharedMemorySize, smem_bytes));
             vf.fn<<<grid, vf.threads, smem_bytes, stream>>>(tp);
             CDH_CUDA(cudaGetLastError());
             ++launches;

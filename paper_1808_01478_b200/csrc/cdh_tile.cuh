@@ -19,7 +19,7 @@ constexpr int kSmemHeader = 128;            // mbarriers + scheduler slot
 constexpr uint64_t kMaxIncrements = 0xFFFFFFFFull;
 
 __host__ __device__ constexpr int tile_smem_bytes(int smem_bins) {
-    return kSmemHeader + 2 * kStageBytes + sizeof(BoxConst) + 16 + 4 * (smem_bins + 1);
+    return kSmemHeader + 2 * kStageBytes + sizeof(BoxConst) + 16 + 4 * (smem_bins + 2);   // + Q3 slot + trash slot
 }
 
 template <int BOX, int TRI, int T, int VAR, bool SPLIT, int MINB>
@@ -45,7 +45,8 @@ __global__ void __launch_bounds__(T, MINB) tile_kernel(const TileParams P) {
     }
 
     if (tid == 0) { mbar_init(bar_addr, 1); mbar_init(bar_addr + 8, 1); fence_mbar_init(); }
-    for (uint32_t b = tid; b <= P.smem_bins; b += T) s_hist[b] = 0;
+    for (uint32_t b = tid; b <= P.smem_bins + 1; b += T) s_hist[b] = 0;
+    const uint32_t trash_addr = hist_addr + 4u * (P.smem_bins + 1u);   // never flushed
     __syncthreads();
 
     uint32_t stage_cnt = 0;                 // stages consumed so far: buffer = cnt & 1, parity = (cnt >> 1) & 1
@@ -185,7 +186,7 @@ __global__ void __launch_bounds__(T, MINB) tile_kernel(const TileParams P) {
                                         d2 = pk2(p, q);
                                     }
                                 }
-                                bin_fast2<SPLIT>(d2, k0, k1, SCALE, ONE, P.thr2_bits, addr_c, hist_addr, sub_c, cur_lim);
+                                bin_fast2<SPLIT>(d2, k0, k1, SCALE, ONE, P.thr2_bits, addr_c, hist_addr, sub_c, cur_lim, trash_addr);
                             }
                         }
                     }
