@@ -75,8 +75,19 @@ inline bool make_box_const(int box_type, const double* box9, double r_max, BoxCo
                 for (int k = -1; k <= 1; ++k, ++m)
                     for (int r = 0; r < 3; ++r)
                         bc->S[m][r] = ((float)i * bc->B[3 * r] + (float)j * bc->B[3 * r + 1]) + (float)k * bc->B[3 * r + 2];
-        // zero-shift candidate alone decides when r_max <= h_min/2
-        bc->prune_ok = (r_max <= 0.5 * h_min * (1.0 + 1e-9)) ? 1.0f : 0.0f;
+        // The zero-shift candidate alone decides when r_max <= h_min/2 and the kernel's
+        // fractional-coordinate test (|s_k - n_k| <= 1/2 - 2^-15) is trustworthy, i.e. the fp32 error of s_k stays
+        // below 2^-16 for |fractional differences| <= 4 (the extent limit of the fast path): that error is bounded
+        // by 40 * 2^-24 * kappa with kappa = max_k sum_c sum_m |Binv[k][c]| |B[c][m]|.
+        double kappa = 0.0;
+        for (int k = 0; k < 3; ++k) {
+            double row = 0.0;
+            for (int c = 0; c < 3; ++c)
+                for (int m = 0; m < 3; ++m) row += std::fabs(Bi[3 * k + c]) * std::fabs(B[3 * c + m]);
+            kappa = std::fmax(kappa, row);
+        }
+        const bool margin_ok = 40.0 * kappa * std::ldexp(1.0, -24) <= std::ldexp(1.0, -16);
+        bc->prune_ok = (r_max <= 0.5 * h_min * (1.0 + 1e-9) && margin_ok) ? 1.0f : 0.0f;
     }
     return true;
 }

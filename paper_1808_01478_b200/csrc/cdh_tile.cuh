@@ -164,29 +164,46 @@ __global__ void __launch_bounds__(T, MINB) tile_kernel(const TileParams P) {
                     } else {
                         const f2 XA = pk2(XJ.x, XJ.y), XB = pk2(XJ.z, XJ.w), YA = pk2(YJ.x, YJ.y), YB = pk2(YJ.z, YJ.w),
                                  ZA = pk2(ZJ.x, ZJ.y), ZB = pk2(ZJ.z, ZJ.w);
+                        // phase 1: the 16 squared distances of this j-group, branch free
+                        f2 D2[kR][2];
+                        float fm[kR][2][2];
+                        float fm_all = 0.0f;
 #pragma unroll
                         for (int r = 0; r < kR; ++r) {
 #pragma unroll
                             for (int hlf = 0; hlf < 2; ++hlf) {
-                                bool nf0, nf1;
-                                f2 d2 = pair_d2_fast<BOX, TRI>(hlf ? XB : XA, hlf ? YB : YA, hlf ? ZB : ZA, xi[r], yi[r], zi[r], fb, ONE, nf0, nf1);
-                                bool k0 = true, k1 = true;
-                                if constexpr (MASKED) { k0 = jg + 2 * hlf > ig + r; k1 = jg + 2 * hlf + 1 > ig + r; }
-                                if constexpr (BOX == BOX_TRI) {
-                                    // zero-shift candidate is decisive unless a fractional coordinate is within
-                                    // kPruneDelta of +-1/2 (or pruning is not allowed for this box / r_max)
-                                    nf0 = (nf0 || !prune) && k0; nf1 = (nf1 || !prune) && k1;
-                                    if (nf0 || nf1) {
-                                        const int c0 = 2 * hlf;
-                                        const float xa = c0 ? XJ.z : XJ.x, ya = c0 ? YJ.z : YJ.x, za = c0 ? ZJ.z : ZJ.x;
-                                        const float xb = c0 ? XJ.w : XJ.y, yb = c0 ? YJ.w : YJ.y, zb = c0 ? ZJ.w : ZJ.y;
-                                        float p, q; upk2(d2, p, q);
-                                        if (nf0) p = pair_d2_simple<BOX_TRI>(xi[r], yi[r], zi[r], xa, ya, za, s_box);
-                                        if (nf1) q = pair_d2_simple<BOX_TRI>(xi[r], yi[r], zi[r], xb, yb, zb, s_box);
-                                        d2 = pk2(p, q);
+                                D2[r][hlf] = pair_d2_fast<BOX, TRI>(hlf ? XB : XA, hlf ? YB : YA, hlf ? ZB : ZA, xi[r], yi[r], zi[r],
+                                                                    fb, ONE, fm[r][hlf][0], fm[r][hlf][1]);
+                                if constexpr (BOX == BOX_TRI) fm_all = fmaxf(fmaxf(fm_all, fm[r][hlf][0]), fm[r][hlf][1]);
+                            }
+                        }
+                        if constexpr (BOX == BOX_TRI) {
+                            // rare: some element of the group has a fractional coordinate within kPruneDelta of
+                            // +-1/2 (or pruning is off for this box / r_max): run the definition for those elements
+                            if (!prune || fm_all > kPruneLimit) {
+                                const float xj[4] = {XJ.x, XJ.y, XJ.z, XJ.w}, yj[4] = {YJ.x, YJ.y, YJ.z, YJ.w}, zj[4] = {ZJ.x, ZJ.y, ZJ.z, ZJ.w};
+#pragma unroll
+                                for (int r = 0; r < kR; ++r) {
+#pragma unroll
+                                    for (int hlf = 0; hlf < 2; ++hlf) {
+                                        float p, q; upk2(D2[r][hlf], p, q);
+                                        bool n0 = !prune || fm[r][hlf][0] > kPruneLimit, n1 = !prune || fm[r][hlf][1] > kPruneLimit;
+                                        if constexpr (MASKED) { n0 = n0 && (jg + 2 * hlf > ig + r); n1 = n1 && (jg + 2 * hlf + 1 > ig + r); }
+                                        if (n0) p = tri_full_d2(xi[r], yi[r], zi[r], xj[2 * hlf], yj[2 * hlf], zj[2 * hlf], s_box);
+                                        if (n1) q = tri_full_d2(xi[r], yi[r], zi[r], xj[2 * hlf + 1], yj[2 * hlf + 1], zj[2 * hlf + 1], s_box);
+                                        D2[r][hlf] = pk2(p, q);
                                     }
                                 }
-                                bin_fast2<SPLIT>(d2, k0, k1, SCALE, ONE, P.thr2_bits, addr_c, hist_addr, sub_c, cur_lim, trash_addr);
+                            }
+                        }
+                        // phase 2: bin and update
+#pragma unroll
+                        for (int r = 0; r < kR; ++r) {
+#pragma unroll
+                            for (int hlf = 0; hlf < 2; ++hlf) {
+                                bool k0 = true, k1 = true;
+                                if constexpr (MASKED) { k0 = jg + 2 * hlf > ig + r; k1 = jg + 2 * hlf + 1 > ig + r; }
+                                bin_fast2<SPLIT>(D2[r][hlf], k0, k1, SCALE, ONE, P.thr2_bits, addr_c, hist_addr, sub_c, cur_lim, trash_addr);
                             }
                         }
                     }
