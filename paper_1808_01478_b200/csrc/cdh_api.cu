@@ -16,7 +16,7 @@ struct cdh_ctx {
     // device scratch, grown on demand, never shrunk
     float* d_pk = nullptr;       size_t pk_bytes = 0;
     void* d_tables = nullptr;    size_t tables_bytes = 0;     // segs | rows | boxes | off | pad_off
-    unsigned int* d_scalars = nullptr;                        // [0] work counter (fast), [1] extent bits, [2] counter (simple)
+    unsigned int* d_scalars = nullptr;                        // [0..2] work counters of the call's tile launches, [4..9] range keys (repack_kernel)
     void* h_tables = nullptr;    size_t h_tables_bytes = 0;   // pinned staging for d_tables
     cudaEvent_t staged = nullptr;                             // h_tables may be rewritten once this has fired
     bool staged_pending = false;
@@ -72,9 +72,10 @@ Variant fast_variant(bool big) {
     return {tile_kernel<BOX, TRI, 256, VAR_FAST, SPLIT, CDH_MINB>, 256};
 }
 template <bool SPLIT>
-Variant pick_fast(int box_type, int tri, bool big) {
+Variant pick_fast(int box_type, int tri, bool big) {      // tri: TRI_* for TRICLINIC, ORTHO_* for ORTHO
     if (box_type == CDH_BOX_NONE) return fast_variant<BOX_NONE, 0, SPLIT>(big);
-    if (box_type == CDH_BOX_ORTHO) return fast_variant<BOX_ORTHO, 0, SPLIT>(big);
+    if (box_type == CDH_BOX_ORTHO)
+        return tri == ORTHO_FUSED ? fast_variant<BOX_ORTHO, ORTHO_FUSED, SPLIT>(big) : fast_variant<BOX_ORTHO, ORTHO_PLAIN, SPLIT>(big);
     if (tri == TRI_UPPER_B01) return fast_variant<BOX_TRI, TRI_UPPER_B01, SPLIT>(big);
     if (tri == TRI_UPPER) return fast_variant<BOX_TRI, TRI_UPPER, SPLIT>(big);
     return fast_variant<BOX_TRI, TRI_GENERAL, SPLIT>(big);
@@ -241,9 +242,30 @@ extern "C" int cdh_histograms(cdh_ctx* ctx, const void* coords, int32_t n_frames
     const int smem_bytes = tile_smem_bytes((int)sp.bins_per_sweep);
     const bool big = 2 * (smem_bytes + 1024) > 228 * 1024;          // one CTA per SM
     const bool split = sp.n_sweeps > 1;
-    bool use_simple_only = (ctx->flags & CDH_FLAG_SIMPLE_KERNEL) != 0 || !(scale_f < 5.0e14f);
-    const Variant vf = split ? pick_fast<true>(box_type, tri, big) : pick_fast<false>(box_type, tri, big);
+    const bool use_simple_only = (ctx->flags & CDH_FLAG_SIMPLE_KERNEL) != 0 || !(scale_f < 5.0e14f);
+    // Launch plan: every tile launch of the call owns an interval (lo, hi] of the fractional-coordinate range the
+    // repack kernel measures, and exactly one of them does the work (cdh_tile.cuh).
+    //   ORTHO: fused rint up to 1.49 (if the host found its constants for every box), magic-number rint up to
+    //          2^20, library rintf beyond;  TRICLINIC: fast path up to 1.49 (n in {-1,0,1}), definition beyond.
+    struct Launch { Variant v; float lo, hi; };
+    const float kInf = INFINITY, kSmall = 1.49f, kMagic = 1048576.0f;
+    bool fused_ok = box_type == CDH_BOX_ORTHO;
+    for (int b = 0; b < nb && fused_ok; ++b) fused_ok = boxes[b].prune_ok != 0.0f;
+    if (ctx->flags & CDH_FLAG_NO_PRUNE) fused_ok = false;          // tests: force the plain magic-number form
+    auto fast_of = [&](int form) { return split ? pick_fast<true>(box_type, form, big) : pick_fast<false>(box_type, form, big); };
     const Variant vs = pick_simple(box_type, big);
+    std::vector<Launch> plan;
+    if (use_simple_only) plan.push_back({vs, -kInf, kInf});
+    else if (box_type == CDH_BOX_NONE) plan.push_back({fast_of(0), -kInf, kInf});
+    else if (box_type == CDH_BOX_ORTHO) {
+        if (fused_ok) { plan.push_back({fast_of(ORTHO_FUSED), -kInf, kSmall}); plan.push_back({fast_of(ORTHO_PLAIN), kSmall, kMagic}); }
+        else plan.push_back({fast_of(ORTHO_PLAIN), -kInf, kMagic});
+        plan.push_back({vs, kMagic, kInf});
+    } else {
+        plan.push_back({fast_of(tri), -kInf, kSmall});
+        plan.push_back({vs, kSmall, kInf});
+    }
+    const Variant vf = plan[0].v;
     const uint32_t ti = (uint32_t)vf.threads * kR;
     CDH_CUDA(cudaFuncSetAttribute((const void*)vf.fn, cudaFuncAttributeMaxDynamicSharedMemorySize, smem_bytes));
     int resident = 0;      // CTAs of the production variant that fit one SM (registers, shared memory)
@@ -292,7 +314,7 @@ extern "C" int cdh_histograms(cdh_ctx* ctx, const void* coords, int32_t n_frames
         rp.coords = (const float*)coords; rp.pk = ctx->d_pk;
         rp.off = (const int32_t*)(d + b_segs + b_rows + b_boxes);
         rp.pad_off = (const uint32_t*)(d + b_segs + b_rows + b_boxes + b_off);
-        rp.extent_bits = ctx->d_scalars + 1;
+        rp.range_keys = ctx->d_scalars + 4;
         rp.boxes = (const BoxConst*)(d + b_segs + b_rows);
         rp.n_species = n_species; rp.n_total = off[n_species]; rp.n_frames = n_frames;
         rp.box_type = box_type; rp.n_boxes = nb > 0 ? nb : 1;
@@ -311,25 +333,16 @@ extern "C" int cdh_histograms(cdh_ctx* ctx, const void* coords, int32_t n_frames
         TileParams tp;
         tp.pk = ctx->d_pk; tp.segs = (const Seg*)d; tp.rows = (const Row*)(d + b_segs);
         tp.boxes = (const BoxConst*)(d + b_segs + b_rows);
-        tp.out = (unsigned long long*)out; tp.extent = (const float*)(ctx->d_scalars + 1);
+        tp.out = (unsigned long long*)out; tp.range_keys = ctx->d_scalars + 4;
         tp.n_rows = (uint32_t)wt.rows.size() - 1; tp.n_items = (uint32_t)wt.n_items;
         tp.n_bins = (uint32_t)n_bins; tp.tj = tj; tp.smem_bins = sp.bins_per_sweep;
         tp.rmax = rmax_f; tp.scale = scale_f; tp.thr2_bits = d2_threshold_bits(rmax_f); tp.one = 1.0f;
-        // fast paths: |b^-1 dx| <= 2 * extent must stay <= 4 (triclinic pruning margin) / 2^21 (magic rint)
-        tp.extent_limit = use_simple_only ? -1.0f : (box_type == CDH_BOX_TRICLINIC ? 2.0f : 1048576.0f);
         grid = grid_full < tp.n_items ? grid_full : tp.n_items;
-        const bool run_fast = !use_simple_only;
-        const bool run_simple = use_simple_only || box_type != CDH_BOX_NONE;
-        if (run_fast) {
-            tp.counter = ctx->d_scalars;
-            vf.fn<<<grid, vf.threads, smem_bytes, stream>>>(tp);
-            CDH_CUDA(cudaGetLastError());
-            ++launches;
-        }
-        if (run_simple) {
-            tp.counter = ctx->d_scalars + 2;
-            CDH_CUDA(cudaFuncSetAttribute((const void*)vs.fn, cudaFuncAttributeMaxDynamicSharedMemorySize, smem_bytes));
-            vs.fn<<<grid, vs.threads, smem_bytes, stream>>>(tp);
+        for (size_t k = 0; k < plan.size(); ++k) {
+            tp.counter = ctx->d_scalars + k;
+            tp.range_lo = plan[k].lo; tp.range_hi = plan[k].hi;
+            if (k > 0) CDH_CUDA(cudaFuncSetAttribute((const void*)plan[k].v.fn, cudaFuncAttributeMaxDynamicSharedMemorySize, smem_bytes));
+            plan[k].v.fn<<<grid, plan[k].v.threads, smem_bytes, stream>>>(tp);
             CDH_CUDA(cudaGetLastError());
             ++launches;
         }

@@ -48,10 +48,11 @@ struct Row {
 // "Host-derived constants").  B has the box vectors as COLUMNS (Eq. 5).
 struct BoxConst {
     float L[3], invL[3];        // ORTHO
+    float invLf[3];             // ORTHO_FUSED: the constant of the fused rint (host search, fused_rint_constant)
     float B[9], Binv[9];        // TRICLINIC, row-major
     float S[27][3];             // TRICLINIC: shift vectors ((i*B[r][0] + j*B[r][1]) + k*B[r][2]), i,j,k in -1..1
     float prune_ok;             // 1: r_max <= h_min/2 with margin, the zero-shift candidate may be tested alone
-    float pad_[2];
+    float pad_[3];
 };
 
 struct TileParams {
@@ -61,7 +62,7 @@ struct TileParams {
     const BoxConst* boxes;
     unsigned int*   counter;    // dynamic work counter (zeroed before the launch)
     unsigned long long* out;    // uint64 [n_hist][n_bins]
-    const float*    extent;     // device scalar written by the repack kernel: max_k |(b^-1 x)_k| over all particles
+    const unsigned int* range_keys;  // device, written by the repack kernel: min / max keys of the fractional coordinates
     uint32_t n_rows, n_items;
     uint32_t n_bins;
     uint32_t tj;                // j-chunk size in particles (multiple of kStageParticles)
@@ -69,7 +70,8 @@ struct TileParams {
     float rmax, scale;          // (float)r_max, (float)(n_bins / r_max)
     uint32_t thr2_bits;         // bits of the smallest fp32 d2 whose correctly rounded sqrt is >= rmax
     float one;                  // 1.0f, opaque to ptxas: keeps packed mul/add pairs unfused
-    float extent_limit;         // fast paths valid while *extent <= extent_limit
+    float range_lo, range_hi;   // periodic boxes: this launch does the work iff range_lo < frac_range() <= range_hi
+                                // (range_hi = +inf: no upper limit, and a NaN range counts as above range_lo)
 };
 
 // ---------------------------------------------------------------------------------------------

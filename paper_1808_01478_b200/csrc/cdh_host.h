@@ -47,6 +47,29 @@ inline bool box_matrices(const double* box9, double B[9], double Bi[9], double* 
     return true;
 }
 
+// Fused rint: the pinned form n = rint(fl(d * invL)) switches from n = 0 to n = 1 at the
+// float c_half = max{c : fl(c * invL) <= 1/2}; the fused form rint(d * invLf) (exact product, one rounding at integer
+// granularity, ties to even) switches at max{c : c * invLf <= 1/2}.  Search the neighbours of invL for an invLf whose
+// switch point is the same float; then both forms agree for every |d| below the 3/2 switch (the kernel's range
+// limit 1.49 keeps |d * invL| well below it).  Products of two floats are exact in double.
+inline bool fused_rint_constant(float invL, float* invLf) {
+    if (!(invL > 0.0f) || !std::isfinite(invL)) return false;
+    auto pinned_zero = [&](float c) { return (float)((double)c * (double)invL) <= 0.5f; };
+    float c = (float)(0.5 / (double)invL);
+    if (!std::isfinite(c) || !(c > 0.0f)) return false;
+    for (int it = 0; it < 64 && !pinned_zero(c); ++it) c = std::nextafterf(c, 0.0f);
+    for (int it = 0; it < 64 && pinned_zero(std::nextafterf(c, INFINITY)); ++it) c = std::nextafterf(c, INFINITY);
+    if (!pinned_zero(c) || pinned_zero(std::nextafterf(c, INFINITY))) return false;
+    const float c_next = std::nextafterf(c, INFINITY);
+    for (int d = 0; d <= 8; ++d)
+        for (int sgn = 1; sgn >= -1; sgn -= 2) {
+            const float cand = bits_f32(f32_bits(invL) + (uint32_t)(sgn * d));
+            if (!(cand > 0.0f) || !std::isfinite(cand)) continue;
+            if ((double)c * (double)cand <= 0.5 && !((double)c_next * (double)cand <= 0.5)) { *invLf = cand; return true; }
+        }
+    return false;
+}
+
 // Fills one BoxConst.  Returns false on an invalid box.
 inline bool make_box_const(int box_type, const double* box9, double r_max, BoxConst* bc) {
     std::memset(bc, 0, sizeof *bc);
@@ -63,7 +86,10 @@ inline bool make_box_const(int box_type, const double* box9, double r_max, BoxCo
             bc->invL[c] = (float)(1.0 / box9[4 * c]);
             if (!std::isfinite(bc->invL[c]) || bc->L[c] == 0.0f) return false;
         }
+        // prune_ok doubles as "fused rint available" for ORTHO (negative box lengths take the plain form)
         bc->prune_ok = 1.0f;
+        for (int c = 0; c < 3; ++c)
+            if (!fused_rint_constant(bc->invL[c], &bc->invLf[c])) { bc->invLf[c] = bc->invL[c]; bc->prune_ok = 0.0f; }
     } else if (box_type == CDH_BOX_TRICLINIC) {
         for (int k = 0; k < 9; ++k) if (!std::isfinite(box9[k])) return false;
         double B[9], Bi[9], h_min;

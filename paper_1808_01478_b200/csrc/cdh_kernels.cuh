@@ -23,6 +23,8 @@ constexpr int BOX_NONE = 0, BOX_ORTHO = 1, BOX_TRI = 2;
 // at most the sign of a zero, never d2): 0 general 3x3, 1 upper triangular (a along x, b in the xy
 // plane), 2 upper triangular with B[0][1] == 0 as well (the rhombic dodecahedron of config 3).
 constexpr int TRI_GENERAL = 0, TRI_UPPER = 1, TRI_UPPER_B01 = 2;
+// For BOX_ORTHO the same template slot selects the rint form: 0 pinned 5-operation form, 1 fused (cdh_fast.cuh).
+constexpr int ORTHO_PLAIN = 0, ORTHO_FUSED = 1;
 
 // ---------------------------------------------------------------------------------------------
 // K0: repack.  One thread per padded particle slot of one frame.
@@ -32,7 +34,8 @@ struct RepackParams {
     float* pk;                  // [n_frames][frame_groups][12]
     const int32_t* off;         // device, [n_species+1] particle offsets
     const uint32_t* pad_off;    // device, [n_species+1] padded particle offsets (multiples of kPadParticles)
-    unsigned int* extent_bits;  // device scalar, atomicMax of the bits of max_k |(b^-1 x)_k| (fractional extent)
+    unsigned int* range_keys;   // device, [6]: atomicMax of key(f_k) (k = 0..2) and of ~key(f_k) (3..5), f = b^-1 x
+                                // (fractional coordinates, approximate); zero-initialised; see frac_range()
     const BoxConst* boxes;      // box constants (periodic boxes), one or n_frames
     int32_t n_species, n_total, n_frames;
     int32_t box_type, n_boxes;
@@ -40,10 +43,30 @@ struct RepackParams {
     uint32_t blocks_per_frame;
 };
 
+// Order-preserving map float -> uint32 (never 0 for a non-NaN float except -NaN patterns, which are excluded).
+__device__ __forceinline__ uint32_t float_key(float v) {
+    const uint32_t b = __float_as_uint(v);
+    return (b & 0x80000000u) ? ~b : (b | 0x80000000u);
+}
+__device__ __forceinline__ float key_float(uint32_t k) {
+    return __uint_as_float((k & 0x80000000u) ? (k & 0x7fffffffu) : ~k);
+}
+// Largest extent over the three axes of the fractional coordinates of all particles of the call (0 if none).
+__device__ __forceinline__ float frac_range(const unsigned int* __restrict__ keys) {
+    float r = 0.0f;
+#pragma unroll
+    for (int q = 0; q < 3; ++q) {
+        const uint32_t kmax = __ldg(keys + q), kmin_c = __ldg(keys + 3 + q);
+        if (kmax != 0u) r = fmaxf(r, key_float(kmax) - key_float(~kmin_c));
+    }
+    return r;
+}
+
 __global__ void __launch_bounds__(256) repack_kernel(const RepackParams P) {
     const uint32_t f = blockIdx.x / P.blocks_per_frame;
     const uint32_t slot = (blockIdx.x % P.blocks_per_frame) * blockDim.x + threadIdx.x;
-    float m = 0.0f;
+    float fr[3] = {0.0f, 0.0f, 0.0f};
+    bool have = false;
     if (slot < P.frame_slots) {
         // species of this slot: largest s with pad_off[s] <= slot
         int lo = 0, hi = P.n_species;
@@ -57,24 +80,35 @@ __global__ void __launch_bounds__(256) repack_kernel(const RepackParams P) {
         if (k < (uint32_t)n) {
             const float* c = P.coords + ((size_t)f * P.n_total + (size_t)__ldg(P.off + lo) + k) * 3;
             x = c[0]; y = c[1]; z = c[2];
-            // Fractional extent |b^-1 x| (approximate, only compared against a limit with a wide margin).
-            // NaN compares false: a NaN coordinate does not raise the extent; its pairs are dropped anyway.
+            // Fractional coordinates b^-1 x (approximate: only their range is compared against limits with wide
+            // margins).  A particle with a NaN coordinate is left out: its pairs are dropped anyway.
             if (P.box_type == BOX_ORTHO) {
                 const BoxConst* bc = P.boxes + (P.n_boxes == 1 ? 0 : f);
-                m = fmaxf(fmaxf(fabsf(x * bc->invL[0]), fabsf(y * bc->invL[1])), fabsf(z * bc->invL[2]));
+                fr[0] = x * bc->invL[0]; fr[1] = y * bc->invL[1]; fr[2] = z * bc->invL[2];
+                have = true;
             } else if (P.box_type == BOX_TRI) {
                 const BoxConst* bc = P.boxes + (P.n_boxes == 1 ? 0 : f);
 #pragma unroll
-                for (int k = 0; k < 3; ++k)
-                    m = fmaxf(m, fabsf(bc->Binv[3 * k] * x + bc->Binv[3 * k + 1] * y + bc->Binv[3 * k + 2] * z));
+                for (int q = 0; q < 3; ++q) fr[q] = bc->Binv[3 * q] * x + bc->Binv[3 * q + 1] * y + bc->Binv[3 * q + 2] * z;
+                have = true;
             }
+            have = have && (fr[0] == fr[0]) && (fr[1] == fr[1]) && (fr[2] == fr[2]);
         }
         float* g = P.pk + ((size_t)f * (P.frame_slots / kGroup) + slot / kGroup) * kGroupFloats + (slot % kGroup);
         g[0] = x; g[4] = y; g[8] = z;
     }
-    // warp max, one atomic per warp (non-negative floats order like their bit patterns)
-    for (int o = 16; o > 0; o >>= 1) m = fmaxf(m, __shfl_xor_sync(0xffffffffu, m, o));
-    if ((threadIdx.x & 31) == 0 && m > 0.0f) atomicMax(P.extent_bits, __float_as_uint(m));
+    if (P.box_type != BOX_NONE) {
+        // warp max / min of the order-preserving keys, two atomics per axis and warp
+#pragma unroll
+        for (int q = 0; q < 3; ++q) {
+            uint32_t kmax = have ? float_key(fr[q]) : 0u, kmin_c = have ? ~float_key(fr[q]) : 0u;
+            for (int o = 16; o > 0; o >>= 1) {
+                kmax = max(kmax, __shfl_xor_sync(0xffffffffu, kmax, o));
+                kmin_c = max(kmin_c, __shfl_xor_sync(0xffffffffu, kmin_c, o));
+            }
+            if ((threadIdx.x & 31) == 0 && kmax != 0u) { atomicMax(P.range_keys + q, kmax); atomicMax(P.range_keys + 3 + q, kmin_c); }
+        }
+    }
 }
 
 // ---------------------------------------------------------------------------------------------

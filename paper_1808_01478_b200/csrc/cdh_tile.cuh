@@ -36,12 +36,13 @@ __global__ void __launch_bounds__(T, MINB) tile_kernel(const TileParams P) {
     const uint32_t stage_addr = smem_u32(stage0);
     const int tid = threadIdx.x;
 
-    // The fast variants are exact only while the coordinate extent keeps |b^-1 dx| small (magic-number
-    // rint, pruning margin); otherwise this launch does nothing and the VAR_SIMPLE launch that follows
-    // it does the work (and vice versa).  Uniform over the grid.
+    // The fast variants are exact only while the range of the fractional coordinates is small (fused rint and
+    // exact B*n: n in {-1,0,1}; magic-number rint: |t| < 2^22).  Every launch of the call reads the range the
+    // repack kernel measured and exactly one of them does the work (no host synchronisation).  Uniform over the grid.
     if constexpr (BOX != BOX_NONE) {
-        const bool fast_ok = __ldg(P.extent) <= P.extent_limit;
-        if ((VAR == VAR_FAST) != fast_ok) return;
+        const float range = frac_range(P.range_keys);
+        const bool mine = !(range <= P.range_lo) && (range <= P.range_hi || P.range_hi == __int_as_float(0x7f800000));
+        if (!mine) return;
     }
 
     if (tid == 0) { mbar_init(bar_addr, 1); mbar_init(bar_addr + 8, 1); fence_mbar_init(); }
@@ -118,7 +119,7 @@ __global__ void __launch_bounds__(T, MINB) tile_kernel(const TileParams P) {
         FastBox fb;
         if constexpr (VAR == VAR_FAST && BOX == BOX_ORTHO) {
 #pragma unroll
-            for (int k = 0; k < 3; ++k) { fb.L[k] = s_box->L[k]; fb.invL[k] = s_box->invL[k]; }
+            for (int k = 0; k < 3; ++k) { fb.L[k] = s_box->L[k]; fb.invL[k] = (TRI == ORTHO_FUSED) ? s_box->invLf[k] : s_box->invL[k]; }
         }
         if constexpr (VAR == VAR_FAST && BOX == BOX_TRI) {
 #pragma unroll

@@ -130,6 +130,39 @@ def test_ortho_unwrapped_coordinates_and_per_frame_boxes():
     assert_same(got, oracle_hist(p), p.name)
 
 
+@pytest.mark.parametrize("seed", [11, 12, 13, 14])
+def test_ortho_awkward_box_lengths_fused_and_plain_rint(seed):
+    # box lengths with full 24-bit mantissas: the fused rint needs a host-searched constant per axis; coordinates
+    # wrapped into the box take the fused form, NO_PRUNE forces the plain magic-number form, both must equal the oracle
+    g = np.random.Generator(np.random.PCG64(seed))
+    L = g.uniform(3.0, 40.0, size=3) * np.array([1.0, 1.0 / 3.0, math.pi])
+    p = inputs.uniform_problem(seed, (1500, 2100), inputs.BOX_ORTHO, 5000, 0.5 * float(L.min()), box=np.diag(L))
+    a, _ = gpu_hist(p)
+    b, _ = gpu_hist(p, cdh.FLAG_NO_PRUNE)
+    assert_same(a, oracle_hist(p), f"fused rint, L={L}")
+    assert_same(b, a, "plain vs fused rint")
+
+
+def test_ortho_pairs_on_the_half_box_switch_point():
+    # separations within a few ulps of L/2 on every axis: where n = rint(d/L) switches between 0 and +-1
+    L = np.array([10.0, 7.3, 12.9])
+    rows = [[0.0, 0.0, 0.0]]
+    for ax in range(3):
+        half = np.float32(L[ax] / 2)
+        for k in range(-6, 7):
+            v = half
+            for _ in range(abs(k)):
+                v = np.nextafter(v, np.float32(np.inf if k > 0 else -np.inf))
+            q = [0.0, 0.0, 0.0]; q[ax] = float(v)
+            rows.append(q)
+    pts = np.array(rows, dtype=np.float32)[None]
+    for r_max in (6.0, 30.0):
+        p = inputs.Problem(f"halfbox{r_max}", pts, np.array([0, 1, len(rows)], dtype=np.int32), inputs.BOX_ORTHO,
+                           np.diag(L).reshape(1, 9), r_max, 1 << 20)
+        got, _ = gpu_hist(p)
+        assert_same(got, oracle_hist(p), p.name)
+
+
 def test_p2_hand_example_species_split():
     pts = np.array([[0, 0, 0], [3, 4, 0], [3, 4, 12], [0, 0, 12]], dtype=np.float32)[None]
     p = inputs.Problem("p2", pts, np.array([0, 2, 4], dtype=np.int32), inputs.BOX_NONE, None, 16.0, 16)
