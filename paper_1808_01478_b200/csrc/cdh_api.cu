@@ -64,12 +64,16 @@ typedef void (*TileFn)(const TileParams);
 struct Variant { TileFn fn; int threads; };
 
 #ifndef CDH_MINB
-#define CDH_MINB 2      // resident CTAs per SM the 256-thread fast variants are register-bounded for
+#define CDH_MINB 3      // resident CTAs per SM the 256-thread NONE / ORTHO fast variants are register-bounded for
+                        // (80 registers; measured +1.5 % over 2; the triclinic variants need 128 registers: 2)
+#endif
+#ifndef CDH_BIG_T
+#define CDH_BIG_T 1024  // threads of the one-CTA-per-SM variants (32 warps/SM: config 5 +5 % over 512)
 #endif
 template <int BOX, int TRI, bool SPLIT>
 Variant fast_variant(bool big) {
-    if (big) return {tile_kernel<BOX, TRI, 512, VAR_FAST, SPLIT, 1>, 512};
-    return {tile_kernel<BOX, TRI, 256, VAR_FAST, SPLIT, CDH_MINB>, 256};
+    if (big) return {tile_kernel<BOX, TRI, CDH_BIG_T, VAR_FAST, SPLIT, 1>, CDH_BIG_T};
+    return {tile_kernel<BOX, TRI, 256, VAR_FAST, SPLIT, (BOX == BOX_TRI ? 2 : CDH_MINB)>, 256};
 }
 template <bool SPLIT>
 Variant pick_fast(int box_type, int tri, bool big) {      // tri: TRI_* for TRICLINIC, ORTHO_* for ORTHO
@@ -82,10 +86,10 @@ Variant pick_fast(int box_type, int tri, bool big) {      // tri: TRI_* for TRIC
 }
 Variant pick_simple(int box_type, bool big) {
     if (box_type == CDH_BOX_NONE)
-        return big ? Variant{tile_kernel<BOX_NONE, 0, 512, VAR_SIMPLE, true, 1>, 512} : Variant{tile_kernel<BOX_NONE, 0, 256, VAR_SIMPLE, true, 2>, 256};
+        return big ? Variant{tile_kernel<BOX_NONE, 0, CDH_BIG_T, VAR_SIMPLE, true, 1>, CDH_BIG_T} : Variant{tile_kernel<BOX_NONE, 0, 256, VAR_SIMPLE, true, 2>, 256};
     if (box_type == CDH_BOX_ORTHO)
-        return big ? Variant{tile_kernel<BOX_ORTHO, 0, 512, VAR_SIMPLE, true, 1>, 512} : Variant{tile_kernel<BOX_ORTHO, 0, 256, VAR_SIMPLE, true, 2>, 256};
-    return big ? Variant{tile_kernel<BOX_TRI, 0, 512, VAR_SIMPLE, true, 1>, 512} : Variant{tile_kernel<BOX_TRI, 0, 256, VAR_SIMPLE, true, 2>, 256};
+        return big ? Variant{tile_kernel<BOX_ORTHO, 0, CDH_BIG_T, VAR_SIMPLE, true, 1>, CDH_BIG_T} : Variant{tile_kernel<BOX_ORTHO, 0, 256, VAR_SIMPLE, true, 2>, 256};
+    return big ? Variant{tile_kernel<BOX_TRI, 0, CDH_BIG_T, VAR_SIMPLE, true, 1>, CDH_BIG_T} : Variant{tile_kernel<BOX_TRI, 0, 256, VAR_SIMPLE, true, 2>, 256};
 }
 
 }  // namespace

@@ -19,7 +19,10 @@ constexpr int kGroupFloats = 12;          // floats per group
 constexpr int kStageParticles = 512;      // j-particles per shared-memory stage (6 KB)
 constexpr int kStageGroups = kStageParticles / kGroup;
 constexpr int kStageBytes = kStageGroups * kGroupFloats * 4;
-constexpr int kPadParticles = 2048;       // multiple of every i-tile size and of kStageParticles
+#ifndef CDH_PAD
+#define CDH_PAD 4096
+#endif
+constexpr int kPadParticles = CDH_PAD;    // multiple of every i-tile size (threads * 4) and of kStageParticles
 
 // One (frame, species pair, bin sweep).  Work items of a segment are (i-tile, j-chunk) pairs.
 struct Seg {

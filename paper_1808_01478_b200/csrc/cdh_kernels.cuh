@@ -98,7 +98,10 @@ __global__ void __launch_bounds__(256) repack_kernel(const RepackParams P) {
         g[0] = x; g[4] = y; g[8] = z;
     }
     if (P.box_type != BOX_NONE) {
-        // warp max / min of the order-preserving keys, two atomics per axis and warp
+        // CTA max / min of the order-preserving keys (shared atomics), then one global atomic per key and CTA
+        __shared__ unsigned int s_keys[6];
+        if (threadIdx.x < 6) s_keys[threadIdx.x] = 0u;
+        __syncthreads();
 #pragma unroll
         for (int q = 0; q < 3; ++q) {
             uint32_t kmax = have ? float_key(fr[q]) : 0u, kmin_c = have ? ~float_key(fr[q]) : 0u;
@@ -106,8 +109,10 @@ __global__ void __launch_bounds__(256) repack_kernel(const RepackParams P) {
                 kmax = max(kmax, __shfl_xor_sync(0xffffffffu, kmax, o));
                 kmin_c = max(kmin_c, __shfl_xor_sync(0xffffffffu, kmin_c, o));
             }
-            if ((threadIdx.x & 31) == 0 && kmax != 0u) { atomicMax(P.range_keys + q, kmax); atomicMax(P.range_keys + 3 + q, kmin_c); }
+            if ((threadIdx.x & 31) == 0 && kmax != 0u) { atomicMax(&s_keys[q], kmax); atomicMax(&s_keys[3 + q], kmin_c); }
         }
+        __syncthreads();
+        if (threadIdx.x < 6 && s_keys[threadIdx.x] != 0u) atomicMax(P.range_keys + threadIdx.x, s_keys[threadIdx.x]);
     }
 }
 
