@@ -37,7 +37,8 @@ extern "C" {
 
 /* precision */
 #define CDH_F32 0              /* the pinned fp32 sequence (built) */
-#define CDH_F64 1              /* SURVEY.md 8(f) "next": returns CDH_ERR_UNSUPPORTED */
+#define CDH_F64 1              /* the same sequence in double (coords are doubles); plain IEEE arithmetic,
+                                  no packed / magic-number shortcuts */
 
 /* return codes */
 #define CDH_OK                 0
@@ -68,7 +69,8 @@ int cdh_create(cdh_ctx **ctx, int device, uint32_t flags);
 /*
  * All species-pair histograms of n_frames frames, summed over the frames.
  *
- *  coords          DEVICE pointer, [n_frames][n_total][3] xyz AoS, contiguous, float (precision CDH_F32).
+ *  coords          DEVICE pointer, [n_frames][n_total][3] xyz AoS, contiguous, float (precision CDH_F32)
+ *                  or double (CDH_F64).
  *                  Coordinates need not be wrapped into the box.  Pairs involving a NaN are dropped.
  *                  Read only during the stream-ordered execution of the call.
  *  n_frames        >= 1.
@@ -84,7 +86,7 @@ int cdh_create(cdh_ctx **ctx, int device, uint32_t flags);
  *  r_max           > 0, finite.  Pairs with !(r < (float)r_max) are dropped in every box mode.
  *  n_bins          1 .. 2^22.  Bin width r_max / n_bins; bin = floor(r * (float)(n_bins / r_max)),
  *                  a kept pair whose product rounds up to n_bins goes to bin n_bins - 1.
- *  precision       CDH_F32.
+ *  precision       CDH_F32 or CDH_F64 (constants are then used in double: r_max, n_bins / r_max, the box).
  *  stream          cudaStream_t (as void*), may be 0.  All work is enqueued on it; the call does not
  *                  synchronise.  `out` is valid once the caller has synchronised the stream.
  *  out             DEVICE pointer, uint64 [n_species*(n_species+1)/2][n_bins], OVERWRITTEN.

@@ -11,14 +11,16 @@ from .binding import (BOX_NONE, BOX_ORTHO, BOX_TRICLINIC, F32, F64, FLAG_MAX_SME
                       cdh_strerror, load)
 
 
-def histograms_device(ctx: "Context", problem, stream=None):
+def histograms_device(ctx: "Context", problem, stream=None, precision: int = F32):
     """Run ``cdh_histograms`` on an ``inputs.Problem``: copies the coordinates to the context's device
     with torch (plumbing), calls the library, returns a torch uint64-as-int64 CUDA tensor [n_hist, n_bins]
-    (not synchronised)."""
+    (not synchronised).  ``precision=F64`` widens the float32 coordinates to double first (exact)."""
+    import numpy as np
     import torch
     dev = torch.device("cuda", ctx.device)
-    coords = torch.from_numpy(problem.coords).to(dev)
+    host = problem.coords.astype(np.float64) if precision == F64 else problem.coords
+    coords = torch.from_numpy(host).to(dev)
     out = torch.empty((problem.n_hist, problem.n_bins), dtype=torch.int64, device=dev)
     ctx.cdh_histograms(coords, problem.n_frames, problem.species_offsets, problem.box_type, problem.box,
-                       problem.r_max, problem.n_bins, out, stream=stream)
+                       problem.r_max, problem.n_bins, out, precision=precision, stream=stream)
     return out

@@ -150,8 +150,9 @@ class Context:
         c = np.ascontiguousarray(coords)
         if c.ndim == 2:
             c = c[None]
-        if c.dtype != np.float32 or c.ndim != 3 or c.shape[2] != 3:
-            raise ValueError("coords must be float32 [n_frames, n_total, 3]")
+        want = np.float64 if precision == F64 else np.float32
+        if c.dtype != want or c.ndim != 3 or c.shape[2] != 3:
+            raise ValueError(f"coords must be {np.dtype(want).name} [n_frames, n_total, 3] for this precision")
         off, b, n_boxes = self._marshal(species_offsets, box, c.shape[0])
         n_species = len(off) - 1
         n_hist = n_species * (n_species + 1) // 2

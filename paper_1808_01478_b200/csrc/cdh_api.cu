@@ -5,6 +5,7 @@
 #include <string>
 #include "cdh_host.h"
 #include "cdh_tile.cuh"
+#include "cdh_f64.cuh"
 
 using namespace cdh;
 
@@ -98,7 +99,7 @@ extern "C" const char* cdh_strerror(int code) {
     switch (code) {
         case CDH_OK: return "ok";
         case CDH_ERR_INVALID_ARG: return "invalid argument";
-        case CDH_ERR_UNSUPPORTED: return "unsupported (precision CDH_F64 is not built)";
+        case CDH_ERR_UNSUPPORTED: return "unsupported";
         case CDH_ERR_ALLOC: return "allocation failed";
         case CDH_ERR_CUDA: return "CUDA runtime error (see cdh_last_error)";
         default: return "unknown error code";
@@ -179,6 +180,132 @@ extern "C" int cdh_destroy(cdh_ctx* ctx) {
     return CDH_OK;
 }
 
+// ---- the double-precision call (cdh_f64.cuh): same layout, tables and stream discipline as the fp32 call --------
+typedef void (*TileFn64)(const TileParams64);
+static inline size_t align256(size_t x) { return (x + 255) & ~(size_t)255; }
+
+static int histograms_f64(cdh_ctx* ctx, const double* coords, int32_t n_frames, const int32_t* off, int32_t n_species,
+                          int32_t box_type, const double* box, int32_t n_boxes, double r_max, int32_t n_bins,
+                          cudaStream_t stream, uint64_t* out) {
+    const int nb = (box_type == CDH_BOX_NONE) ? 0 : n_boxes;
+    std::vector<BoxConst64> boxes((size_t)(nb > 0 ? nb : 1));
+    std::memset(boxes.data(), 0, boxes.size() * sizeof(BoxConst64));
+    for (int b = 0; b < nb; ++b) {
+        if (!make_box_const64(box_type, box + 9 * (size_t)b, r_max, &boxes[b])) return CDH_ERR_INVALID_ARG;
+        if (ctx->flags & CDH_FLAG_NO_PRUNE) boxes[b].prune_ok = 0.0;
+    }
+    std::vector<uint32_t> pad_off((size_t)n_species + 1);
+    uint64_t slots = 0;
+    for (int s = 0; s < n_species; ++s) {
+        pad_off[s] = (uint32_t)slots;
+        const uint64_t n = (uint64_t)(off[s + 1] - off[s]);
+        slots += (n + kPadParticles - 1) / kPadParticles * kPadParticles;
+        if (slots > 0x7fffffffull) return CDH_ERR_INVALID_ARG;
+    }
+    pad_off[n_species] = (uint32_t)slots;
+    const uint32_t frame_slots = (uint32_t)slots;
+    if ((uint64_t)frame_slots * (uint64_t)n_frames / kGroup > 0xffffffffull) return CDH_ERR_INVALID_ARG;
+    const int n_hist = n_species * (n_species + 1) / 2;
+
+    DeviceGuard guard(ctx->device);
+    if (!guard.ok) return cuda_fail(ctx, cudaGetLastError(), "cudaSetDevice");
+
+    uint32_t cap_bins = (uint32_t)((ctx->max_smem_optin - tile_smem_bytes64(0)) / 4);
+    const uint32_t flag_cap = ctx->flags >> CDH_FLAG_MAX_SMEM_BINS_SHIFT;
+    if (flag_cap && flag_cap < cap_bins) cap_bins = flag_cap;
+    const SweepPlan sp = plan_sweeps((uint32_t)n_bins, cap_bins);
+    const int smem_bytes = tile_smem_bytes64((int)sp.bins_per_sweep);
+    const bool big = 2 * (smem_bytes + 1024) > 228 * 1024;
+    TileFn64 fn; int threads;
+    if (box_type == CDH_BOX_NONE) { fn = big ? tile_kernel_f64<BOX_NONE, 512, 1> : tile_kernel_f64<BOX_NONE, 256, 2>; }
+    else if (box_type == CDH_BOX_ORTHO) { fn = big ? tile_kernel_f64<BOX_ORTHO, 512, 1> : tile_kernel_f64<BOX_ORTHO, 256, 2>; }
+    else { fn = big ? tile_kernel_f64<BOX_TRI, 512, 1> : tile_kernel_f64<BOX_TRI, 256, 2>; }
+    threads = big ? 512 : 256;
+    const uint32_t ti = (uint32_t)threads * kR;
+    CDH_CUDA(cudaFuncSetAttribute((const void*)fn, cudaFuncAttributeMaxDynamicSharedMemorySize, smem_bytes));
+    int resident = 0;
+    CDH_CUDA(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&resident, (const void*)fn, threads, (size_t)smem_bytes));
+    if (resident < 1) resident = 1;
+    const uint32_t grid_full = (uint32_t)ctx->n_sm * (uint32_t)resident;
+
+    WorkTables wt;
+    uint32_t tj = 8192;
+    for (;; tj >>= 1) {
+        build_tables(n_frames, off, n_species, nb > 0 ? nb : 1, (uint32_t)n_bins, sp, ti, tj, pad_off, frame_slots, &wt);
+        if (wt.n_items >= 16ull * grid_full || tj == (uint32_t)kStageParticles) break;
+    }
+    if (wt.n_items >= 0xffffffffull || wt.rows.size() >= 0x7fffffffull) return CDH_ERR_INVALID_ARG;
+
+    const size_t b_segs = align256(wt.segs.size() * sizeof(Seg) + 1), b_rows = align256(wt.rows.size() * sizeof(Row)),
+                 b_boxes = align256(boxes.size() * sizeof(BoxConst64)), b_off = align256(((size_t)n_species + 1) * 4);
+    const size_t tables = b_segs + b_rows + b_boxes + 2 * b_off;
+    int rc;
+    if (ctx->staged_pending) { CDH_CUDA(cudaEventSynchronize(ctx->staged)); ctx->staged_pending = false; }
+    if ((rc = grow(ctx, &ctx->h_tables, &ctx->h_tables_bytes, tables, true)) != CDH_OK) return rc;
+    if ((rc = grow(ctx, &ctx->d_tables, &ctx->tables_bytes, tables, false)) != CDH_OK) return rc;
+    const size_t pk_need = (size_t)n_frames * frame_slots * 3 * sizeof(double);
+    if ((rc = grow(ctx, (void**)&ctx->d_pk, &ctx->pk_bytes, pk_need > 0 ? pk_need : 16, false)) != CDH_OK) return rc;
+
+    char* h = (char*)ctx->h_tables;
+    std::memcpy(h, wt.segs.data(), wt.segs.size() * sizeof(Seg));
+    std::memcpy(h + b_segs, wt.rows.data(), wt.rows.size() * sizeof(Row));
+    std::memcpy(h + b_segs + b_rows, boxes.data(), boxes.size() * sizeof(BoxConst64));
+    std::memcpy(h + b_segs + b_rows + b_boxes, off, ((size_t)n_species + 1) * 4);
+    std::memcpy(h + b_segs + b_rows + b_boxes + b_off, pad_off.data(), ((size_t)n_species + 1) * 4);
+    char* d = (char*)ctx->d_tables;
+    const bool timing = ctx->ev != nullptr;
+    cudaEvent_t* ev = timing ? ctx->ev + 4 * (ctx->timed_calls % CDH_TIMED_CALLS) : nullptr;
+    if (timing) CDH_CUDA(cudaEventRecord(ev[0], stream));
+    CDH_CUDA(cudaMemcpyAsync(d, h, tables, cudaMemcpyHostToDevice, stream));
+    CDH_CUDA(cudaEventRecord(ctx->staged, stream));
+    ctx->staged_pending = true;
+    CDH_CUDA(cudaMemsetAsync(ctx->d_scalars, 0, 64, stream));
+    CDH_CUDA(cudaMemsetAsync(out, 0, (size_t)n_hist * (size_t)n_bins * sizeof(uint64_t), stream));
+
+    int launches = 0;
+    if (frame_slots > 0) {
+        RepackParams64 rp;
+        rp.coords = coords; rp.pk = (double*)ctx->d_pk;
+        rp.off = (const int32_t*)(d + b_segs + b_rows + b_boxes);
+        rp.pad_off = (const uint32_t*)(d + b_segs + b_rows + b_boxes + b_off);
+        rp.range_keys = ctx->d_scalars + 4;
+        rp.boxes = (const BoxConst64*)(d + b_segs + b_rows);
+        rp.n_species = n_species; rp.n_total = off[n_species]; rp.n_frames = n_frames;
+        rp.box_type = box_type; rp.n_boxes = nb > 0 ? nb : 1;
+        rp.frame_slots = frame_slots; rp.blocks_per_frame = (frame_slots + 255) / 256;
+        const uint64_t blocks = (uint64_t)rp.blocks_per_frame * (uint64_t)n_frames;
+        if (blocks > 0x7fffffffull) return CDH_ERR_INVALID_ARG;
+        repack_kernel_f64<<<(unsigned)blocks, 256, 0, stream>>>(rp);
+        CDH_CUDA(cudaGetLastError());
+        ++launches;
+    }
+    uint32_t grid = 0;
+    if (timing) CDH_CUDA(cudaEventRecord(ev[1], stream));
+    if (wt.n_items > 0) {
+        TileParams64 tp;
+        tp.pk = (const double*)ctx->d_pk; tp.segs = (const Seg*)d; tp.rows = (const Row*)(d + b_segs);
+        tp.boxes = (const BoxConst64*)(d + b_segs + b_rows);
+        tp.counter = ctx->d_scalars; tp.out = (unsigned long long*)out; tp.range_keys = ctx->d_scalars + 4;
+        tp.n_rows = (uint32_t)wt.rows.size() - 1; tp.n_items = (uint32_t)wt.n_items;
+        tp.n_bins = (uint32_t)n_bins; tp.tj = tj; tp.smem_bins = sp.bins_per_sweep;
+        tp.rmax = r_max; tp.scale = (double)n_bins / r_max;
+        grid = grid_full < tp.n_items ? grid_full : tp.n_items;
+        fn<<<grid, threads, smem_bytes, stream>>>(tp);
+        CDH_CUDA(cudaGetLastError());
+        ++launches;
+    }
+    if (timing) {
+        CDH_CUDA(cudaEventRecord(ev[2], stream));
+        CDH_CUDA(cudaEventRecord(ev[3], stream));
+        ++ctx->timed_calls;
+    }
+    ctx->info[0] = launches; ctx->info[1] = (int64_t)wt.n_items; ctx->info[2] = sp.n_sweeps; ctx->info[3] = grid;
+    ctx->info[4] = threads; ctx->info[5] = smem_bytes;
+    ctx->info[6] = 2 | (box_type << 4) | ((int)(sp.n_sweeps > 1) << 12) | ((int)big << 13) | ((int64_t)tj << 16);
+    ctx->info[7] = (int64_t)wt.padded_pairs;
+    return CDH_OK;
+}
+
 static int validate(const void* coords, int32_t n_frames, const int32_t* off, int32_t n_species, int32_t box_type,
                     const double* box, int32_t n_boxes, double r_max, int32_t n_bins, int32_t precision, const void* out) {
     if (!coords || !off || !out) return CDH_ERR_INVALID_ARG;
@@ -194,11 +321,8 @@ static int validate(const void* coords, int32_t n_frames, const int32_t* off, in
     if (!((float)r_max > 0.0f) || !std::isfinite((float)r_max)) return CDH_ERR_INVALID_ARG;
     const float scale = (float)((double)n_bins / r_max);
     if (!std::isfinite(scale) || !(scale > 0.0f)) return CDH_ERR_INVALID_ARG;
-    if (precision == CDH_F64) return CDH_ERR_UNSUPPORTED;
     return CDH_OK;
 }
-
-static inline size_t align256(size_t x) { return (x + 255) & ~(size_t)255; }
 
 extern "C" int cdh_histograms(cdh_ctx* ctx, const void* coords, int32_t n_frames, const int32_t* off,
                               int32_t n_species, int32_t box_type, const double* box, int32_t n_boxes,
@@ -208,6 +332,8 @@ extern "C" int cdh_histograms(cdh_ctx* ctx, const void* coords, int32_t n_frames
     if (rc != CDH_OK) return rc;
     cudaStream_t stream = (cudaStream_t)stream_;
     ctx->err.clear();
+    if (precision == CDH_F64)
+        return histograms_f64(ctx, (const double*)coords, n_frames, off, n_species, box_type, box, n_boxes, r_max, n_bins, stream, out);
 
     // ---- host-derived constants ----------------------------------------------------------------
     const int nb = (box_type == CDH_BOX_NONE) ? 0 : n_boxes;
@@ -372,7 +498,7 @@ extern "C" int cdh_histograms_host(cdh_ctx* ctx, const void* coords, int32_t n_f
     cudaStream_t stream = (cudaStream_t)stream_;
     DeviceGuard guard(ctx->device);
     if (!guard.ok) return cuda_fail(ctx, cudaGetLastError(), "cudaSetDevice");
-    const size_t cbytes = (size_t)n_frames * (size_t)off[n_species] * 3 * sizeof(float);
+    const size_t cbytes = (size_t)n_frames * (size_t)off[n_species] * 3 * (precision == CDH_F64 ? sizeof(double) : sizeof(float));
     const size_t obytes = (size_t)(n_species * (n_species + 1) / 2) * (size_t)n_bins * sizeof(uint64_t);
     if ((rc = grow(ctx, &ctx->d_io_coords, &ctx->io_coords_bytes, cbytes > 0 ? cbytes : 16, false)) != CDH_OK) return rc;
     if ((rc = grow(ctx, &ctx->d_io_out, &ctx->io_out_bytes, obytes, false)) != CDH_OK) return rc;

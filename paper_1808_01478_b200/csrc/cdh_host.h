@@ -8,6 +8,7 @@
 #include <cstring>
 #include <vector>
 #include "cdh_device.cuh"
+#include "cdh_f64.cuh"
 #include "../../include/cdh.h"
 
 namespace cdh {
@@ -114,6 +115,46 @@ inline bool make_box_const(int box_type, const double* box9, double r_max, BoxCo
         }
         const bool margin_ok = 15.0 * kappa * std::ldexp(1.0, -24) <= std::ldexp(1.0, -18);
         bc->prune_ok = (r_max <= 0.5 * h_min * (1.0 + 1e-9) && margin_ok) ? 1.0f : 0.0f;
+    }
+    return true;
+}
+
+// The same constants for the double-precision path (T = double: no rounding after the double derivation).
+inline bool make_box_const64(int box_type, const double* box9, double r_max, BoxConst64* bc) {
+    std::memset(bc, 0, sizeof *bc);
+    if (box_type == CDH_BOX_ORTHO) {
+        for (int r = 0; r < 3; ++r)
+            for (int c = 0; c < 3; ++c) {
+                const double v = box9[3 * r + c];
+                if (!std::isfinite(v)) return false;
+                if (r != c && v != 0.0) return false;
+                if (r == c && v == 0.0) return false;
+            }
+        for (int c = 0; c < 3; ++c) {
+            bc->L[c] = box9[4 * c];
+            bc->invL[c] = 1.0 / box9[4 * c];
+            if (!std::isfinite(bc->invL[c])) return false;
+        }
+    } else if (box_type == CDH_BOX_TRICLINIC) {
+        for (int k = 0; k < 9; ++k) if (!std::isfinite(box9[k])) return false;
+        double h_min;
+        if (!box_matrices(box9, bc->B, bc->Binv, &h_min)) return false;
+        int m = 0;
+        for (int i = -1; i <= 1; ++i)
+            for (int j = -1; j <= 1; ++j)
+                for (int k = -1; k <= 1; ++k, ++m)
+                    for (int r = 0; r < 3; ++r)
+                        bc->S[m][r] = ((double)i * bc->B[3 * r] + (double)j * bc->B[3 * r + 1]) + (double)k * bc->B[3 * r + 2];
+        // pruning: |s_k - n_k| <= 1/2 - 2^-30 is trustworthy while the double error of
+        // s_k (<= 15 * 2^-53 * kappa * range, range <= 1024 checked on the device) stays below 2^-31: kappa <= 256.
+        double kappa = 0.0;
+        for (int k = 0; k < 3; ++k) {
+            double row = 0.0;
+            for (int c = 0; c < 3; ++c)
+                for (int q = 0; q < 3; ++q) row += std::fabs(bc->Binv[3 * k + c]) * std::fabs(bc->B[3 * c + q]);
+            kappa = std::fmax(kappa, row);
+        }
+        bc->prune_ok = (r_max <= 0.5 * h_min * (1.0 + 1e-12) && kappa <= 256.0) ? 1.0 : 0.0;   // slack << the 2^-30 margin
     }
     return true;
 }

@@ -168,7 +168,7 @@ __global__ void __launch_bounds__(T, MINB) tile_kernel(const TileParams P) {
                         // phase 1: the 16 squared distances of this j-group, branch free
                         f2 D2[kR][2];
                         float fm[kR][2][2];
-                        float fm_all = 0.0f;
+                        [[maybe_unused]] float fm_all = 0.0f;
 #pragma unroll
                         for (int r = 0; r < kR; ++r) {
 #pragma unroll

@@ -1,0 +1,98 @@
+"""-m gpu: the double-precision path (precision CDH_F64) against the fp64 oracle, bin for bin.
+
+Both sides run the pinned sequence in IEEE double; the float32 coordinates of the seeded
+generators are widened to double exactly, so the histograms must be identical integers.
+"""
+import math
+
+import numpy as np
+import pytest
+
+import paper_1808_01478_b200 as cdh
+from paper_1808_01478_b200 import inputs
+from oracle import oracle as cdh_oracle
+
+torch = pytest.importorskip("torch")
+pytestmark = pytest.mark.gpu
+
+
+def gpu64(p, flags=0):
+    if not torch.cuda.is_available():
+        pytest.skip("no CUDA device")
+    with cdh.Context(0, flags) as ctx:
+        out = cdh.histograms_device(ctx, p, precision=cdh.F64)
+        torch.cuda.synchronize()
+        return out.cpu().numpy().view(np.uint64), ctx.last_call_info()
+
+
+def oracle64(p):
+    return cdh_oracle.histograms(p.coords.astype(np.float64), p.species_offsets, p.box_type, p.box, p.r_max, p.n_bins,
+                                 precision="f64")
+
+
+def same(got, want, what):
+    if not np.array_equal(got, want):
+        d = got.astype(np.int64) - want.astype(np.int64)
+        raise AssertionError(f"{what}: {np.count_nonzero(d)} bins differ, L1 = {int(np.abs(d).sum())}, "
+                             f"sums {int(got.sum())} / {int(want.sum())}")
+
+
+@pytest.mark.parametrize("k", [1, 2, 3, 4, 5])
+def test_reduced_configs_f64_bit_exact(k):
+    p = inputs.reduced_config(k)
+    got, info = gpu64(p)
+    same(got, oracle64(p), f"{p.name} f64 {info}")
+
+
+def test_f64_split_path_and_no_prune():
+    p = inputs.reduced_config(3)
+    want = oracle64(p)
+    a, info = gpu64(p, 4000 << cdh.FLAG_MAX_SMEM_BINS_SHIFT)
+    assert info["sweeps"] == 5
+    same(a, want, "f64 bin-range split")
+    b, _ = gpu64(p, cdh.FLAG_NO_PRUNE)
+    same(b, want, "f64 27-shift search everywhere")
+
+
+def test_f64_general_box_beyond_half_height_and_outside_coordinates():
+    box = np.array([[9.0, 0.5, -0.25], [1.5, 8.0, 0.75], [-2.0, 2.5, 7.0]])
+    for spread, r_max in ((1.0, 2.5), (3.5, 2.5), (1.0, 5.5)):
+        p = inputs.uniform_problem(91, (700, 900), inputs.BOX_TRICLINIC, 3000, r_max, box=box, spread=spread)
+        got, _ = gpu64(p)
+        same(got, oracle64(p), f"general box spread={spread} r_max={r_max}")
+
+
+def test_f64_hand_examples_and_total_count():
+    pts = np.array([[1, 1, 1], [8, 8, 2], [2, 14, 9], [13, 3, 15]], dtype=np.float32)[None]
+    box = np.array([[16.0, 0, 0], [0, 16.0, 0], [8.0, 8.0, 16.0]]).reshape(1, 9)
+    p = inputs.Problem("p4", pts, np.array([0, 4], dtype=np.int32), inputs.BOX_TRICLINIC, box, 16.0, 16)
+    got, _ = gpu64(p)
+    want = np.zeros((1, 16), dtype=np.uint64); want[0, 5] = 1; want[0, 7] = 1; want[0, 8] = 1; want[0, 9] = 3   # pin P4
+    same(got, want, "P4 in double")
+    q = inputs.config1()
+    got, _ = gpu64(q)
+    assert int(got.sum()) == 1_999_000
+    same(got, oracle64(q), "config 1 in double")
+
+
+def test_f64_differs_from_f32_only_by_adjacent_bin_moves():
+    if not torch.cuda.is_available():
+        pytest.skip("no CUDA device")
+    p = inputs.reduced_config(2)
+    with cdh.Context(0) as ctx:
+        a = cdh.histograms_device(ctx, p).cpu().numpy().astype(np.int64)
+        b = cdh.histograms_device(ctx, p, precision=cdh.F64).cpu().numpy().astype(np.int64)
+    assert abs(int(a.sum()) - int(b.sum())) <= 8                     # pairs within a few ulp of r_max
+    cum = np.abs(np.cumsum(a - b, axis=1))
+    assert cum.max() <= 64                                           # moves between neighbouring bins only
+    assert 0 < np.abs(a - b).sum() < 4 * p.n_bins * 2.0 ** -24 * p.evaluated_pairs * 2   # SURVEY.md 8c model bound
+
+
+def test_f64_host_entry_point():
+    if not torch.cuda.is_available():
+        pytest.skip("no CUDA device")
+    p = inputs.reduced_config(4)
+    with cdh.Context(0) as ctx:
+        got = ctx.cdh_histograms_host(p.coords.astype(np.float64), p.species_offsets, p.box_type, p.box, p.r_max, p.n_bins,
+                                      precision=cdh.F64)
+    same(got, oracle64(p), "cdh_histograms_host in double")

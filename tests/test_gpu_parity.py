@@ -244,8 +244,8 @@ def test_argument_errors_leave_out_untouched():
                 ctx.cdh_histograms(coords, 1, p.species_offsets, p.box_type, None, args["r_max"], args["n_bins"], out)
             assert e.value.code == cdh.binding.ERR_INVALID_ARG
         with pytest.raises(cdh.CdhError) as e:
-            ctx.cdh_histograms(coords, 1, p.species_offsets, p.box_type, None, p.r_max, p.n_bins, out, precision=cdh.F64)
-        assert e.value.code == cdh.binding.ERR_UNSUPPORTED
+            ctx.cdh_histograms(coords, 1, p.species_offsets, p.box_type, None, p.r_max, p.n_bins, out, precision=7)
+        assert e.value.code == cdh.binding.ERR_INVALID_ARG
         with pytest.raises(cdh.CdhError):       # singular box
             ctx.cdh_histograms(coords, 1, p.species_offsets, inputs.BOX_TRICLINIC, np.zeros((1, 9)), 1.0, 10, out)
         with pytest.raises(cdh.CdhError):       # off-diagonal with ORTHO
