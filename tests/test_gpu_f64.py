@@ -96,3 +96,10 @@ def test_f64_host_entry_point():
         got = ctx.cdh_histograms_host(p.coords.astype(np.float64), p.species_offsets, p.box_type, p.box, p.r_max, p.n_bins,
                                       precision=cdh.F64)
     same(got, oracle64(p), "cdh_histograms_host in double")
+
+
+def test_f64_config2_full_size():
+    p = inputs.config2()
+    got, info = gpu64(p)
+    same(got, oracle64(p), f"config 2 full size in double {info}")
+    assert got.sum() / p.evaluated_pairs == pytest.approx(math.pi / 6, rel=2e-3)
