@@ -52,8 +52,10 @@ extern "C" {
 #define CDH_FLAG_SIMPLE_KERNEL   (1u << 0) /* plain scalar kernel with library sqrtf/rintf/floorf: the
                                               cross-validation kernel */
 #define CDH_FLAG_NO_PRUNE        (1u << 1) /* triclinic: always search the 27 shifts */
-#define CDH_FLAG_WARP_AGGREGATE  (1u << 2) /* always aggregate equal bins in a warp (__match_any_sync) */
-#define CDH_FLAG_NO_AGGREGATE    (1u << 3) /* never aggregate */
+#define CDH_FLAG_WARP_AGGREGATE  (1u << 2) /* plain kernel, equal bins of a warp aggregated in software
+                                              (__match_any_sync, one ATOMS.ADD per distinct bin) */
+#define CDH_FLAG_NO_AGGREGATE    (1u << 3) /* plain kernel, one ATOMS.ADD per lane (no aggregation at all);
+                                              production uses ATOMS.POPC.INC, which merges equal addresses in hardware */
 #define CDH_FLAG_TIME_KERNELS     (1u << 4) /* record CUDA events around the tile kernel(s) of every call
                                               (measurement; read with cdh_last_call_kernel_ms) */
 #define CDH_FLAG_MAX_SMEM_BINS_SHIFT 8     /* bits 8..31: if non-zero, cap on the bins one CTA keeps in

@@ -85,12 +85,18 @@ Variant pick_fast(int box_type, int tri, bool big) {      // tri: TRI_* for TRIC
     if (tri == TRI_UPPER) return fast_variant<BOX_TRI, TRI_UPPER, SPLIT>(big);
     return fast_variant<BOX_TRI, TRI_GENERAL, SPLIT>(big);
 }
-Variant pick_simple(int box_type, bool big) {
+template <int VAR>
+Variant simple_variant(int box_type, bool big) {
     if (box_type == CDH_BOX_NONE)
-        return big ? Variant{tile_kernel<BOX_NONE, 0, CDH_BIG_T, VAR_SIMPLE, true, 1>, CDH_BIG_T} : Variant{tile_kernel<BOX_NONE, 0, 256, VAR_SIMPLE, true, 2>, 256};
+        return big ? Variant{tile_kernel<BOX_NONE, 0, CDH_BIG_T, VAR, true, 1>, CDH_BIG_T} : Variant{tile_kernel<BOX_NONE, 0, 256, VAR, true, 2>, 256};
     if (box_type == CDH_BOX_ORTHO)
-        return big ? Variant{tile_kernel<BOX_ORTHO, 0, CDH_BIG_T, VAR_SIMPLE, true, 1>, CDH_BIG_T} : Variant{tile_kernel<BOX_ORTHO, 0, 256, VAR_SIMPLE, true, 2>, 256};
-    return big ? Variant{tile_kernel<BOX_TRI, 0, CDH_BIG_T, VAR_SIMPLE, true, 1>, CDH_BIG_T} : Variant{tile_kernel<BOX_TRI, 0, 256, VAR_SIMPLE, true, 2>, 256};
+        return big ? Variant{tile_kernel<BOX_ORTHO, 0, CDH_BIG_T, VAR, true, 1>, CDH_BIG_T} : Variant{tile_kernel<BOX_ORTHO, 0, 256, VAR, true, 2>, 256};
+    return big ? Variant{tile_kernel<BOX_TRI, 0, CDH_BIG_T, VAR, true, 1>, CDH_BIG_T} : Variant{tile_kernel<BOX_TRI, 0, 256, VAR, true, 2>, 256};
+}
+Variant pick_simple(int box_type, bool big, uint32_t flags) {
+    if (flags & CDH_FLAG_WARP_AGGREGATE) return simple_variant<VAR_SIMPLE_MATCH>(box_type, big);
+    if (flags & CDH_FLAG_NO_AGGREGATE) return simple_variant<VAR_SIMPLE_PLAIN>(box_type, big);
+    return simple_variant<VAR_SIMPLE>(box_type, big);
 }
 
 }  // namespace
@@ -372,7 +378,8 @@ extern "C" int cdh_histograms(cdh_ctx* ctx, const void* coords, int32_t n_frames
     const int smem_bytes = tile_smem_bytes((int)sp.bins_per_sweep);
     const bool big = 2 * (smem_bytes + 1024) > 228 * 1024;          // one CTA per SM
     const bool split = sp.n_sweeps > 1;
-    const bool use_simple_only = (ctx->flags & CDH_FLAG_SIMPLE_KERNEL) != 0 || !(scale_f < 5.0e14f);
+    const bool use_simple_only = (ctx->flags & (CDH_FLAG_SIMPLE_KERNEL | CDH_FLAG_WARP_AGGREGATE | CDH_FLAG_NO_AGGREGATE)) != 0 ||
+                                 !(scale_f < 5.0e14f);
     // Launch plan: every tile launch of the call owns an interval (lo, hi] of the fractional-coordinate range the
     // repack kernel measures, and exactly one of them does the work (cdh_tile.cuh).
     //   ORTHO: fused rint up to 1.49 (if the host found its constants for every box), magic-number rint up to
@@ -383,7 +390,7 @@ extern "C" int cdh_histograms(cdh_ctx* ctx, const void* coords, int32_t n_frames
     for (int b = 0; b < nb && fused_ok; ++b) fused_ok = boxes[b].prune_ok != 0.0f;
     if (ctx->flags & CDH_FLAG_NO_PRUNE) fused_ok = false;          // tests: force the plain magic-number form
     auto fast_of = [&](int form) { return split ? pick_fast<true>(box_type, form, big) : pick_fast<false>(box_type, form, big); };
-    const Variant vs = pick_simple(box_type, big);
+    const Variant vs = pick_simple(box_type, big, ctx->flags);
     std::vector<Launch> plan;
     if (use_simple_only) plan.push_back({vs, -kInf, kInf});
     else if (box_type == CDH_BOX_NONE) plan.push_back({fast_of(0), -kInf, kInf});

@@ -16,6 +16,11 @@ namespace cdh {
 
 constexpr int VAR_SIMPLE = 0;
 constexpr int VAR_FAST = 1;
+// Two more forms of the plain kernel's histogram update, for measuring what the hardware merge of equal addresses in
+// ATOMS.POPC.INC is worth: software aggregation of equal bins with __match_any_sync
+// and one ATOMS.ADD per distinct bin (CDH_FLAG_WARP_AGGREGATE), and one ATOMS.ADD per lane (CDH_FLAG_NO_AGGREGATE).
+constexpr int VAR_SIMPLE_MATCH = 2;
+constexpr int VAR_SIMPLE_PLAIN = 3;
 
 constexpr int BOX_NONE = 0, BOX_ORTHO = 1, BOX_TRI = 2;
 
@@ -161,15 +166,26 @@ __device__ __forceinline__ float pair_d2_simple(float xi, float yi, float zi, fl
 }
 
 // Binning of one d2 by the pinned sequence (library sqrt / floor).  hist = shared address of slot 0,
-// the CTA owns bins [bin_lo, bin_lo + lim).
-__device__ __forceinline__ void bin_simple(float d2, float rmax, float scale, uint32_t n_bins,
+// the CTA owns bins [bin_lo, bin_lo + lim).  Must be called by all 32 lanes of the warp (keep = false for a pair
+// that does not exist): the VAR_SIMPLE_MATCH form synchronises the warp.
+template <int VAR>
+__device__ __forceinline__ void bin_simple(float d2, bool keep, float rmax, float scale, uint32_t n_bins,
                                            uint32_t hist, uint32_t bin_lo, uint32_t lim) {
     const float d = __fsqrt_rn(d2);
-    if (d < rmax) {                                       // drops d >= r_max and NaN
-        uint32_t b = (uint32_t)floorf(__fmul_rn(d, scale));
-        b = min(b, n_bins - 1u);                          // reading Q3
-        b -= bin_lo;
-        if (b < lim) hist_inc(hist + 4u * b);
+    keep = keep && (d < rmax);                            // drops d >= r_max and NaN
+    uint32_t b = 0xFFFFFFFFu;
+    if (keep) {
+        b = (uint32_t)fminf(floorf(__fmul_rn(d, scale)), 4294967040.0f);
+        b = min(b, n_bins - 1u) - bin_lo;                 // reading Q3; unsigned wrap for bins below the sweep
+        if (!(b < lim)) b = 0xFFFFFFFFu;
+    }
+    if constexpr (VAR == VAR_SIMPLE_MATCH) {
+        const uint32_t peers = __match_any_sync(0xffffffffu, b);
+        if (b != 0xFFFFFFFFu && (uint32_t)(__ffs(peers) - 1) == (threadIdx.x & 31u)) hist_add(hist + 4u * b, (uint32_t)__popc(peers));
+    } else if constexpr (VAR == VAR_SIMPLE_PLAIN) {
+        if (b != 0xFFFFFFFFu) hist_add(hist + 4u * b, 1u + (n_bins >> 31));     // a register operand: ATOMS.ADD, not POPC.INC
+    } else {
+        if (b != 0xFFFFFFFFu) hist_inc(hist + 4u * b);
     }
 }
 

@@ -152,15 +152,15 @@ __global__ void __launch_bounds__(T, MINB) tile_kernel(const TileParams P) {
                 for (uint32_t g = 0; g < n_grp; ++g) {
                     const float4 XJ = sj[3 * g], YJ = sj[3 * g + 1], ZJ = sj[3 * g + 2];
                     const uint32_t jg = jbase + 4u * g;
-                    if constexpr (VAR == VAR_SIMPLE) {
+                    if constexpr (VAR != VAR_FAST) {
                         const float xj[4] = {XJ.x, XJ.y, XJ.z, XJ.w}, yj[4] = {YJ.x, YJ.y, YJ.z, YJ.w}, zj[4] = {ZJ.x, ZJ.y, ZJ.z, ZJ.w};
 #pragma unroll
                         for (int c = 0; c < 4; ++c)
 #pragma unroll
                             for (int r = 0; r < kR; ++r) {
-                                if (MASKED && !(jg + c > ig + r)) continue;
+                                const bool keep = !MASKED || (jg + c > ig + r);
                                 const float d2 = pair_d2_simple<BOX>(xi[r], yi[r], zi[r], xj[c], yj[c], zj[c], s_box);
-                                bin_simple(d2, P.rmax, P.scale, P.n_bins, hist_addr, cur_lo, cur_lim);
+                                bin_simple<VAR>(d2, keep, P.rmax, P.scale, P.n_bins, hist_addr, cur_lo, cur_lim);
                             }
                     } else {
                         const f2 XA = pk2(XJ.x, XJ.y), XB = pk2(XJ.z, XJ.w), YA = pk2(YJ.x, YJ.y), YB = pk2(YJ.z, YJ.w),

@@ -59,6 +59,8 @@ FLAG_SETS = {
     "simple": cdh.FLAG_SIMPLE_KERNEL,
     "split3000": 3000 << cdh.FLAG_MAX_SMEM_BINS_SHIFT,
     "simple_split700": cdh.FLAG_SIMPLE_KERNEL | (700 << cdh.FLAG_MAX_SMEM_BINS_SHIFT),
+    "match_any": cdh.FLAG_WARP_AGGREGATE,
+    "plain_add": cdh.FLAG_NO_AGGREGATE,
 }
 
 
