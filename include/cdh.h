@@ -58,6 +58,8 @@ extern "C" {
                                               production uses ATOMS.POPC.INC, which merges equal addresses in hardware */
 #define CDH_FLAG_TIME_KERNELS     (1u << 4) /* record CUDA events around the tile kernel(s) of every call
                                               (measurement; read with cdh_last_call_kernel_ms) */
+#define CDH_FLAG_GLOBAL_HIST      (1u << 5) /* no private histogram: every kept pair adds to the uint64 result
+                                              directly (chosen automatically for very wide histograms) */
 #define CDH_FLAG_MAX_SMEM_BINS_SHIFT 8     /* bits 8..31: if non-zero, cap on the bins one CTA keeps in
                                               shared memory (forces the bin-range-split path) */
 

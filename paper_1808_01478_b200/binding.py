@@ -24,6 +24,7 @@ FLAG_NO_PRUNE = 1 << 1
 FLAG_WARP_AGGREGATE = 1 << 2
 FLAG_NO_AGGREGATE = 1 << 3
 FLAG_TIME_KERNELS = 1 << 4
+FLAG_GLOBAL_HIST = 1 << 5
 FLAG_MAX_SMEM_BINS_SHIFT = 8
 
 EXPORTS = ["cdh_create", "cdh_histograms", "cdh_histograms_host", "cdh_destroy", "cdh_strerror",
@@ -170,7 +171,7 @@ class Context:
         self._check(self._lib.cdh_last_call_info(self._h, arr))
         v = list(arr)
         return {"launches": v[0], "items": v[1], "sweeps": v[2], "ctas": v[3], "threads": v[4],
-                "smem_bytes": v[5], "variant": v[6], "tj": v[6] >> 16, "fast": bool(v[6] & 1),
+                "smem_bytes": v[5], "variant": v[6], "tj": v[6] >> 16, "fast": bool(v[6] & 1), "global_hist": bool(v[6] & 4),
                 "padded_pairs": v[7]}
 
     def call_kernel_ms(self, calls_back: int = 0):

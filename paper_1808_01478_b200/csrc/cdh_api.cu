@@ -64,6 +64,11 @@ int grow(cdh_ctx* ctx, void** p, size_t* have, size_t need, bool pinned_host) {
 typedef void (*TileFn)(const TileParams);
 struct Variant { TileFn fn; int threads; };
 
+#ifndef CDH_GLOBAL_SWEEPS
+#define CDH_GLOBAL_SWEEPS 8   // shared-memory sweeps from which the global-histogram mode takes over (measured
+                              // break-even: 200,000 uniform points, 400,000 bins: 8 sweeps 200 vs global 221 Gpairs/s)
+#endif
+constexpr uint32_t kGlobalSweeps = CDH_GLOBAL_SWEEPS;
 #ifndef CDH_MINB
 #define CDH_MINB 3      // resident CTAs per SM the 256-thread NONE / ORTHO fast variants are register-bounded for
                         // (80 registers; measured +1.5 % over 2; the triclinic variants need 128 registers: 2)
@@ -71,12 +76,13 @@ struct Variant { TileFn fn; int threads; };
 #ifndef CDH_BIG_T
 #define CDH_BIG_T 1024  // threads of the one-CTA-per-SM variants (32 warps/SM: config 5 +5 % over 512)
 #endif
-template <int BOX, int TRI, bool SPLIT>
+template <int BOX, int TRI, int MODE>
 Variant fast_variant(bool big) {
-    if (big) return {tile_kernel<BOX, TRI, CDH_BIG_T, VAR_FAST, SPLIT, 1>, CDH_BIG_T};
-    return {tile_kernel<BOX, TRI, 256, VAR_FAST, SPLIT, (BOX == BOX_TRI ? 2 : CDH_MINB)>, 256};
+    if constexpr (MODE != MODE_GLOBAL)
+        if (big) return {tile_kernel<BOX, TRI, CDH_BIG_T, VAR_FAST, MODE, 1>, CDH_BIG_T};
+    return {tile_kernel<BOX, TRI, 256, VAR_FAST, MODE, (BOX == BOX_TRI ? 2 : CDH_MINB)>, 256};
 }
-template <bool SPLIT>
+template <int SPLIT>
 Variant pick_fast(int box_type, int tri, bool big) {      // tri: TRI_* for TRICLINIC, ORTHO_* for ORTHO
     if (box_type == CDH_BOX_NONE) return fast_variant<BOX_NONE, 0, SPLIT>(big);
     if (box_type == CDH_BOX_ORTHO)
@@ -88,10 +94,15 @@ Variant pick_fast(int box_type, int tri, bool big) {      // tri: TRI_* for TRIC
 template <int VAR>
 Variant simple_variant(int box_type, bool big) {
     if (box_type == CDH_BOX_NONE)
-        return big ? Variant{tile_kernel<BOX_NONE, 0, CDH_BIG_T, VAR, true, 1>, CDH_BIG_T} : Variant{tile_kernel<BOX_NONE, 0, 256, VAR, true, 2>, 256};
+        return big ? Variant{tile_kernel<BOX_NONE, 0, CDH_BIG_T, VAR, MODE_SPLIT, 1>, CDH_BIG_T} : Variant{tile_kernel<BOX_NONE, 0, 256, VAR, MODE_SPLIT, 2>, 256};
     if (box_type == CDH_BOX_ORTHO)
-        return big ? Variant{tile_kernel<BOX_ORTHO, 0, CDH_BIG_T, VAR, true, 1>, CDH_BIG_T} : Variant{tile_kernel<BOX_ORTHO, 0, 256, VAR, true, 2>, 256};
-    return big ? Variant{tile_kernel<BOX_TRI, 0, CDH_BIG_T, VAR, true, 1>, CDH_BIG_T} : Variant{tile_kernel<BOX_TRI, 0, 256, VAR, true, 2>, 256};
+        return big ? Variant{tile_kernel<BOX_ORTHO, 0, CDH_BIG_T, VAR, MODE_SPLIT, 1>, CDH_BIG_T} : Variant{tile_kernel<BOX_ORTHO, 0, 256, VAR, MODE_SPLIT, 2>, 256};
+    return big ? Variant{tile_kernel<BOX_TRI, 0, CDH_BIG_T, VAR, MODE_SPLIT, 1>, CDH_BIG_T} : Variant{tile_kernel<BOX_TRI, 0, 256, VAR, MODE_SPLIT, 2>, 256};
+}
+Variant simple_global(int box_type) {
+    if (box_type == CDH_BOX_NONE) return {tile_kernel<BOX_NONE, 0, 256, VAR_SIMPLE, MODE_GLOBAL, 2>, 256};
+    if (box_type == CDH_BOX_ORTHO) return {tile_kernel<BOX_ORTHO, 0, 256, VAR_SIMPLE, MODE_GLOBAL, 2>, 256};
+    return {tile_kernel<BOX_TRI, 0, 256, VAR_SIMPLE, MODE_GLOBAL, 2>, 256};
 }
 Variant pick_simple(int box_type, bool big, uint32_t flags) {
     if (flags & CDH_FLAG_WARP_AGGREGATE) return simple_variant<VAR_SIMPLE_MATCH>(box_type, big);
@@ -374,8 +385,12 @@ extern "C" int cdh_histograms(cdh_ctx* ctx, const void* coords, int32_t n_frames
     uint32_t cap_bins = (uint32_t)((ctx->max_smem_optin - tile_smem_bytes(0)) / 4);
     const uint32_t flag_cap = ctx->flags >> CDH_FLAG_MAX_SMEM_BINS_SHIFT;
     if (flag_cap && flag_cap < cap_bins) cap_bins = flag_cap;
-    const SweepPlan sp = plan_sweeps((uint32_t)n_bins, cap_bins);
-    const int smem_bytes = tile_smem_bytes((int)sp.bins_per_sweep);
+    SweepPlan sp = plan_sweeps((uint32_t)n_bins, cap_bins);
+    // Very wide histograms (the paper's global-memory kernel regime): beyond kGlobalSweeps
+    // sweeps the private copy is dropped and updates go straight to the uint64 result in L2 (MODE_GLOBAL).
+    const bool global_hist = (ctx->flags & CDH_FLAG_GLOBAL_HIST) != 0 || (!flag_cap && sp.n_sweeps >= kGlobalSweeps);
+    if (global_hist) { sp.n_sweeps = 1; sp.bins_per_sweep = (uint32_t)n_bins; }
+    const int smem_bytes = tile_smem_bytes(global_hist ? 0 : (int)sp.bins_per_sweep);
     const bool big = 2 * (smem_bytes + 1024) > 228 * 1024;          // one CTA per SM
     const bool split = sp.n_sweeps > 1;
     const bool use_simple_only = (ctx->flags & (CDH_FLAG_SIMPLE_KERNEL | CDH_FLAG_WARP_AGGREGATE | CDH_FLAG_NO_AGGREGATE)) != 0 ||
@@ -389,8 +404,11 @@ extern "C" int cdh_histograms(cdh_ctx* ctx, const void* coords, int32_t n_frames
     bool fused_ok = box_type == CDH_BOX_ORTHO;
     for (int b = 0; b < nb && fused_ok; ++b) fused_ok = boxes[b].prune_ok != 0.0f;
     if (ctx->flags & CDH_FLAG_NO_PRUNE) fused_ok = false;          // tests: force the plain magic-number form
-    auto fast_of = [&](int form) { return split ? pick_fast<true>(box_type, form, big) : pick_fast<false>(box_type, form, big); };
-    const Variant vs = pick_simple(box_type, big, ctx->flags);
+    auto fast_of = [&](int form) {
+        return global_hist ? pick_fast<MODE_GLOBAL>(box_type, form, big)
+                           : split ? pick_fast<MODE_SPLIT>(box_type, form, big) : pick_fast<MODE_SHARED>(box_type, form, big);
+    };
+    const Variant vs = global_hist ? simple_global(box_type) : pick_simple(box_type, big, ctx->flags);
     std::vector<Launch> plan;
     if (use_simple_only) plan.push_back({vs, -kInf, kInf});
     else if (box_type == CDH_BOX_NONE) plan.push_back({fast_of(0), -kInf, kInf});
@@ -472,7 +490,7 @@ extern "C" int cdh_histograms(cdh_ctx* ctx, const void* coords, int32_t n_frames
         tp.boxes = (const BoxConst*)(d + b_segs + b_rows);
         tp.out = (unsigned long long*)out; tp.range_keys = ctx->d_scalars + 4;
         tp.n_rows = (uint32_t)wt.rows.size() - 1; tp.n_items = (uint32_t)wt.n_items;
-        tp.n_bins = (uint32_t)n_bins; tp.tj = tj; tp.smem_bins = sp.bins_per_sweep;
+        tp.n_bins = (uint32_t)n_bins; tp.tj = tj; tp.smem_bins = global_hist ? 0u : sp.bins_per_sweep;
         tp.rmax = rmax_f; tp.scale = scale_f; tp.thr2_bits = d2_threshold_bits(rmax_f); tp.one = 1.0f;
         grid = grid_full < tp.n_items ? grid_full : tp.n_items;
         for (size_t k = 0; k < plan.size(); ++k) {
@@ -491,7 +509,7 @@ extern "C" int cdh_histograms(cdh_ctx* ctx, const void* coords, int32_t n_frames
     }
     ctx->info[0] = launches; ctx->info[1] = (int64_t)wt.n_items; ctx->info[2] = sp.n_sweeps; ctx->info[3] = grid;
     ctx->info[4] = vf.threads; ctx->info[5] = smem_bytes;
-    ctx->info[6] = (use_simple_only ? 0 : 1) | (box_type << 4) | (tri << 8) | ((int)split << 12) | ((int)big << 13) | ((int64_t)tj << 16);
+    ctx->info[6] = (use_simple_only ? 0 : 1) | ((int)global_hist << 2) | (box_type << 4) | (tri << 8) | ((int)split << 12) | ((int)big << 13) | ((int64_t)tj << 16);
     ctx->info[7] = (int64_t)wt.padded_pairs;
     return CDH_OK;
 }

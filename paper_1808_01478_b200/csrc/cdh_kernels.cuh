@@ -24,6 +24,10 @@ constexpr int VAR_SIMPLE_PLAIN = 3;
 
 constexpr int BOX_NONE = 0, BOX_ORTHO = 1, BOX_TRI = 2;
 
+// Where the histogram lives: one shared-memory copy of all bins; a shared copy of one bin range per sweep; no private
+// copy at all, updates go straight to the uint64 result in L2 (very wide histograms).
+constexpr int MODE_SHARED = 0, MODE_SPLIT = 1, MODE_GLOBAL = 2;
+
 // Triclinic zero structure (skipping a term whose matrix entry is exactly 0 in B and in B^-1 changes
 // at most the sign of a zero, never d2): 0 general 3x3, 1 upper triangular (a along x, b in the xy
 // plane), 2 upper triangular with B[0][1] == 0 as well (the rhombic dodecahedron of config 3).
@@ -168,9 +172,9 @@ __device__ __forceinline__ float pair_d2_simple(float xi, float yi, float zi, fl
 // Binning of one d2 by the pinned sequence (library sqrt / floor).  hist = shared address of slot 0,
 // the CTA owns bins [bin_lo, bin_lo + lim).  Must be called by all 32 lanes of the warp (keep = false for a pair
 // that does not exist): the VAR_SIMPLE_MATCH form synchronises the warp.
-template <int VAR>
+template <int VAR, int MODE>
 __device__ __forceinline__ void bin_simple(float d2, bool keep, float rmax, float scale, uint32_t n_bins,
-                                           uint32_t hist, uint32_t bin_lo, uint32_t lim) {
+                                           uint32_t hist, uint32_t bin_lo, uint32_t lim, unsigned long long* __restrict__ grow) {
     const float d = __fsqrt_rn(d2);
     keep = keep && (d < rmax);                            // drops d >= r_max and NaN
     uint32_t b = 0xFFFFFFFFu;
@@ -179,7 +183,9 @@ __device__ __forceinline__ void bin_simple(float d2, bool keep, float rmax, floa
         b = min(b, n_bins - 1u) - bin_lo;                 // reading Q3; unsigned wrap for bins below the sweep
         if (!(b < lim)) b = 0xFFFFFFFFu;
     }
-    if constexpr (VAR == VAR_SIMPLE_MATCH) {
+    if constexpr (MODE == MODE_GLOBAL) {
+        if (b != 0xFFFFFFFFu) atomicAdd(grow + b, 1ull);      // bin_lo = 0, lim = n_bins + 1 in this mode
+    } else if constexpr (VAR == VAR_SIMPLE_MATCH) {
         const uint32_t peers = __match_any_sync(0xffffffffu, b);
         if (b != 0xFFFFFFFFu && (uint32_t)(__ffs(peers) - 1) == (threadIdx.x & 31u)) hist_add(hist + 4u * b, (uint32_t)__popc(peers));
     } else if constexpr (VAR == VAR_SIMPLE_PLAIN) {

@@ -22,7 +22,7 @@ __host__ __device__ constexpr int tile_smem_bytes(int smem_bins) {
     return kSmemHeader + 2 * kStageBytes + sizeof(BoxConst) + 16 + 4 * (smem_bins + 2);   // + Q3 slot + trash slot
 }
 
-template <int BOX, int TRI, int T, int VAR, bool SPLIT, int MINB>
+template <int BOX, int TRI, int T, int VAR, int MODE, int MINB>
 __global__ void __launch_bounds__(T, MINB) tile_kernel(const TileParams P) {
     extern __shared__ __align__(128) unsigned char smem[];
     constexpr int TI = T * kR;
@@ -58,7 +58,7 @@ __global__ void __launch_bounds__(T, MINB) tile_kernel(const TileParams P) {
 
     auto flush = [&]() {
         __syncthreads();
-        if (cur_key != 0xFFFFFFFFu) {
+        if (MODE != MODE_GLOBAL && cur_key != 0xFFFFFFFFu) {
             unsigned long long* o = P.out + (size_t)cur_hist * P.n_bins;
             for (uint32_t b = tid; b < cur_lim; b += T) {
                 const uint32_t v = s_hist[b];
@@ -128,6 +128,7 @@ __global__ void __launch_bounds__(T, MINB) tile_kernel(const TileParams P) {
         const bool prune = (BOX == BOX_TRI) ? (s_box->prune_ok != 0.0f) : true;
         const uint32_t addr_c = hist_addr - 4u * (kFloorMagicBits + cur_lo);
         const uint32_t sub_c = kFloorMagicBits + cur_lo;
+        unsigned long long* const grow = P.out + (size_t)seg.hist * P.n_bins;     // MODE_GLOBAL: the result row itself
 
         if (tid == 0 && s_begin < n_stage) {
             const uint32_t b = stage_cnt & 1u;
@@ -160,7 +161,7 @@ __global__ void __launch_bounds__(T, MINB) tile_kernel(const TileParams P) {
                             for (int r = 0; r < kR; ++r) {
                                 const bool keep = !MASKED || (jg + c > ig + r);
                                 const float d2 = pair_d2_simple<BOX>(xi[r], yi[r], zi[r], xj[c], yj[c], zj[c], s_box);
-                                bin_simple<VAR>(d2, keep, P.rmax, P.scale, P.n_bins, hist_addr, cur_lo, cur_lim);
+                                bin_simple<VAR, MODE>(d2, keep, P.rmax, P.scale, P.n_bins, hist_addr, cur_lo, cur_lim, grow);
                             }
                     } else {
                         const f2 XA = pk2(XJ.x, XJ.y), XB = pk2(XJ.z, XJ.w), YA = pk2(YJ.x, YJ.y), YB = pk2(YJ.z, YJ.w),
@@ -204,7 +205,7 @@ __global__ void __launch_bounds__(T, MINB) tile_kernel(const TileParams P) {
                             for (int hlf = 0; hlf < 2; ++hlf) {
                                 bool k0 = true, k1 = true;
                                 if constexpr (MASKED) { k0 = jg + 2 * hlf > ig + r; k1 = jg + 2 * hlf + 1 > ig + r; }
-                                bin_fast2<SPLIT>(D2[r][hlf], k0, k1, SCALE, ONE, P.thr2_bits, addr_c, hist_addr, sub_c, cur_lim, trash_addr);
+                                bin_fast2<MODE>(D2[r][hlf], k0, k1, SCALE, ONE, P.thr2_bits, addr_c, hist_addr, sub_c, cur_lim, trash_addr, grow, P.n_bins - 1u);
                             }
                         }
                     }

@@ -59,6 +59,8 @@ FLAG_SETS = {
     "simple": cdh.FLAG_SIMPLE_KERNEL,
     "split3000": 3000 << cdh.FLAG_MAX_SMEM_BINS_SHIFT,
     "simple_split700": cdh.FLAG_SIMPLE_KERNEL | (700 << cdh.FLAG_MAX_SMEM_BINS_SHIFT),
+    "global_hist": cdh.FLAG_GLOBAL_HIST,
+    "simple_global_hist": cdh.FLAG_GLOBAL_HIST | cdh.FLAG_SIMPLE_KERNEL,
     "match_any": cdh.FLAG_WARP_AGGREGATE,
     "plain_add": cdh.FLAG_NO_AGGREGATE,
 }
@@ -195,11 +197,20 @@ def test_p8_single_bin_exceeds_uint32():
     assert int(got[0, 0]) == 4_999_950_000 and int(got.sum()) == 4_999_950_000
 
 
-def test_p9_wide_bin_split():
+def test_p9_wide_histogram_global_and_split_paths():
+    # 1,000,000 bins = 4 MB >> shared memory: the global-histogram mode takes over by itself; a cap on the shared
+    # bins forces the bin-range-split path (20 sweeps) instead; both must equal the oracle
     p = inputs.uniform_problem(9, (6000,), inputs.BOX_NONE, 1_000_000, math.sqrt(3.0))
     got, info = gpu_hist(p)
-    assert info["sweeps"] > 1
-    assert_same(got, oracle_hist(p), f"1M bins {info}")
+    assert info["global_hist"] and info["sweeps"] == 1
+    assert_same(got, oracle_hist(p), f"1M bins, global histogram {info}")
+    got, info = gpu_hist(p, 50000 << cdh.FLAG_MAX_SMEM_BINS_SHIFT)
+    assert not info["global_hist"] and info["sweeps"] == 20
+    assert_same(got, oracle_hist(p), f"1M bins, 20 sweeps {info}")
+    q = inputs.uniform_problem(10, (2500, 3000), inputs.BOX_ORTHO, 400_000, 3.0, box=np.diag([6.0, 7.0, 8.0]))
+    got, info = gpu_hist(q)
+    assert info["global_hist"]
+    assert_same(got, oracle_hist(q), f"400k bins orthorhombic, global histogram {info}")
 
 
 def test_empty_species_tiny_inputs_and_nan():
