@@ -140,6 +140,19 @@ int cdh_last_call_info(const cdh_ctx *ctx, int64_t info[8]);
 #define CDH_TIMED_CALLS 256
 int cdh_call_kernel_ms(cdh_ctx *ctx, int calls_back, double ms[2]);
 
+/*
+ * Radial distribution function from a summed histogram (Eqs. 1-3):
+ *   p_kappa = hist[kappa] / n_frames,   g_kappa = p_kappa / (4 pi (n_pairs / volume) r^2 dr),
+ *   dr = r_max / n_bins,  r = (kappa + 1/2) dr  (bin centre).  IEEE double, operations in this order.
+ *  hist     DEVICE, uint64 [n_hist][n_bins] (the result of cdh_histograms).
+ *  n_pairs  HOST, [n_hist]: unique pairs per frame behind each histogram (N(N-1)/2 or N1*N2); 0 gives inf / NaN rows.
+ *  volume   system volume V > 0;  n_frames >= 1: the frames that were summed into hist.
+ *  g        DEVICE, double [n_hist][n_bins], overwritten.  Asynchronous on `stream`.
+ * Returns CDH_OK, CDH_ERR_INVALID_ARG (nothing enqueued), CDH_ERR_ALLOC or CDH_ERR_CUDA.
+ */
+int cdh_rdf(cdh_ctx *ctx, const uint64_t *hist, int32_t n_hist, int32_t n_bins, double r_max, int32_t n_frames,
+            const double *n_pairs, double volume, void *stream, double *g);
+
 #ifdef __cplusplus
 }
 #endif

@@ -265,3 +265,29 @@ int cdh_oracle_max_threads(void)
     return 1;
 #endif
 }
+
+/* ------------------------------- g(r) post-processing ------------------------------------- */
+/* Radial distribution function from a summed histogram, Eqs. 1-3:
+ *   p_kappa = hist[kappa] / N_frames                     (Eq. 2/3: average number of pairs in the bin per frame)
+ *   g_kappa = p_kappa / (4 pi (N_pairs / V) r^2 dr)      (Eq. 1 with dr = bin width r_max / n_bins and r taken at
+ *                                                         the bin centre (kappa + 1/2) dr -- reading Q15)
+ * n_pairs[h] is the number of unique pairs per frame behind histogram h, volume the system volume V.
+ * Plain double arithmetic in the order written (no contraction).  Returns 0, or -1 on bad arguments. */
+int cdh_oracle_rdf(const uint64_t *hist, int n_hist, int n_bins, double r_max, int n_frames,
+                   const double *n_pairs, double volume, double *g)
+{
+    if (!hist || !n_pairs || !g || n_hist < 1 || n_bins < 1 || n_frames < 1 || !(r_max > 0.0) || !(volume > 0.0))
+        return -1;
+    const double dr = r_max / (double)n_bins;
+    const double four_pi = 4.0 * 3.14159265358979323846;
+    for (int h = 0; h < n_hist; ++h) {
+        const double density = n_pairs[h] / volume;
+        for (int k = 0; k < n_bins; ++k) {
+            const double r = ((double)k + 0.5) * dr;
+            const double shell = (four_pi * (r * r)) * dr;
+            const double p = (double)hist[(size_t)h * (size_t)n_bins + (size_t)k] / (double)n_frames;
+            g[(size_t)h * (size_t)n_bins + (size_t)k] = p / (density * shell);
+        }
+    }
+    return 0;
+}

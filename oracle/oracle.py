@@ -41,6 +41,9 @@ def _load():
         lib.cdh_oracle_pair_d2.restype = ctypes.c_double
         lib.cdh_oracle_pair_d2.argtypes = [ctypes.c_void_p, ctypes.c_void_p, ctypes.c_int,
                                            ctypes.c_void_p, ctypes.c_int]
+        lib.cdh_oracle_rdf.restype = ctypes.c_int
+        lib.cdh_oracle_rdf.argtypes = [ctypes.c_void_p, ctypes.c_int, ctypes.c_int, ctypes.c_double, ctypes.c_int,
+                                       ctypes.c_void_p, ctypes.c_double, ctypes.c_void_p]
         lib.cdh_oracle_max_threads.restype = ctypes.c_int
         _lib = lib
     return _lib
@@ -98,3 +101,20 @@ def pair_d2(pi, pj, box_type: int, box: Optional[np.ndarray], precision: str = "
     return float(lib.cdh_oracle_pair_d2(a.ctypes.data, b.ctypes.data, int(box_type),
                                         None if bx is None else bx.ctypes.data,
                                         {"f32": 0, "f64": 1}[precision]))
+
+
+def rdf(hist: np.ndarray, r_max: float, n_frames: int, n_pairs, volume: float) -> np.ndarray:
+    """g(r) per histogram row from summed uint64 counts (Eqs. 1-3); float64 [n_hist, n_bins]."""
+    lib = _load()
+    h = np.ascontiguousarray(hist, dtype=np.uint64)
+    if h.ndim == 1:
+        h = h[None]
+    npairs = np.ascontiguousarray(n_pairs, dtype=np.float64).reshape(-1)
+    if npairs.shape[0] != h.shape[0]:
+        raise ValueError("one pair count per histogram row")
+    g = np.empty(h.shape, dtype=np.float64)
+    rc = lib.cdh_oracle_rdf(h.ctypes.data, h.shape[0], h.shape[1], float(r_max), int(n_frames), npairs.ctypes.data,
+                            float(volume), g.ctypes.data)
+    if rc != 0:
+        raise ValueError("cdh_oracle_rdf rejected its arguments")
+    return g

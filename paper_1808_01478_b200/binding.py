@@ -28,7 +28,7 @@ FLAG_GLOBAL_HIST = 1 << 5
 FLAG_MAX_SMEM_BINS_SHIFT = 8
 
 EXPORTS = ["cdh_create", "cdh_histograms", "cdh_histograms_host", "cdh_destroy", "cdh_strerror",
-           "cdh_last_error", "cdh_last_call_info", "cdh_call_kernel_ms",
+           "cdh_last_error", "cdh_last_call_info", "cdh_call_kernel_ms", "cdh_rdf",
            "cdh_bench_fp32_rate", "cdh_bench_shared_atomics", "cdh_selftest_sqrt"]
 
 
@@ -69,6 +69,8 @@ def load(path: Optional[str] = None) -> ctypes.CDLL:
     lib.cdh_last_call_info.argtypes = [vp, ctypes.POINTER(ctypes.c_int64)]
     lib.cdh_call_kernel_ms.restype = ctypes.c_int
     lib.cdh_call_kernel_ms.argtypes = [vp, ctypes.c_int, ctypes.POINTER(dbl)]
+    lib.cdh_rdf.restype = ctypes.c_int
+    lib.cdh_rdf.argtypes = [vp, vp, i32, i32, dbl, i32, vp, dbl, vp, vp]
     lib.cdh_bench_fp32_rate.restype = ctypes.c_int
     lib.cdh_bench_fp32_rate.argtypes = [ctypes.c_int, ctypes.c_int, vp, ctypes.POINTER(dbl), ctypes.POINTER(dbl)]
     lib.cdh_bench_shared_atomics.restype = ctypes.c_int
@@ -165,6 +167,16 @@ class Context:
                                            out.ctypes.data)
         self._check(rc)
         return out
+
+    def cdh_rdf(self, hist, n_hist: int, n_bins: int, r_max: float, n_frames: int, n_pairs, volume: float, g,
+                stream=None) -> None:
+        """include/cdh.h ``cdh_rdf``: hist (uint64) and g (float64) are DEVICE buffers [n_hist, n_bins]."""
+        npairs = np.ascontiguousarray(n_pairs, dtype=np.float64).reshape(-1)
+        if npairs.shape[0] != int(n_hist):
+            raise ValueError("one pair count per histogram row")
+        rc = self._lib.cdh_rdf(self._h, _ptr(hist), int(n_hist), int(n_bins), float(r_max), int(n_frames),
+                               npairs.ctypes.data, float(volume), _stream_ptr(stream), _ptr(g))
+        self._check(rc)
 
     def last_call_info(self) -> dict:
         arr = (ctypes.c_int64 * 8)()

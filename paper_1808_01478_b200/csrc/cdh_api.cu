@@ -6,6 +6,7 @@
 #include "cdh_host.h"
 #include "cdh_tile.cuh"
 #include "cdh_f64.cuh"
+#include "cdh_rdf.cuh"
 
 using namespace cdh;
 
@@ -533,5 +534,35 @@ extern "C" int cdh_histograms_host(cdh_ctx* ctx, const void* coords, int32_t n_f
     if (rc != CDH_OK) return rc;
     CDH_CUDA(cudaMemcpyAsync(out, ctx->d_io_out, obytes, cudaMemcpyDeviceToHost, stream));                      // one D2H copy
     CDH_CUDA(cudaStreamSynchronize(stream));
+    return CDH_OK;
+}
+
+extern "C" int cdh_rdf(cdh_ctx* ctx, const uint64_t* hist, int32_t n_hist, int32_t n_bins, double r_max, int32_t n_frames,
+                       const double* n_pairs, double volume, void* stream_, double* g) {
+    if (!ctx || !hist || !n_pairs || !g || n_hist < 1 || n_bins < 1 || n_frames < 1) return CDH_ERR_INVALID_ARG;
+    if (!(r_max > 0.0) || !std::isfinite(r_max) || !(volume > 0.0) || !std::isfinite(volume)) return CDH_ERR_INVALID_ARG;
+    for (int h = 0; h < n_hist; ++h) if (!(n_pairs[h] >= 0.0) || !std::isfinite(n_pairs[h])) return CDH_ERR_INVALID_ARG;
+    cudaStream_t stream = (cudaStream_t)stream_;
+    ctx->err.clear();
+    DeviceGuard guard(ctx->device);
+    if (!guard.ok) return cuda_fail(ctx, cudaGetLastError(), "cudaSetDevice");
+    int rc;
+    const size_t bytes = (size_t)n_hist * sizeof(double);
+    if (ctx->staged_pending) { CDH_CUDA(cudaEventSynchronize(ctx->staged)); ctx->staged_pending = false; }
+    if ((rc = grow(ctx, &ctx->h_tables, &ctx->h_tables_bytes, bytes, true)) != CDH_OK) return rc;
+    if ((rc = grow(ctx, &ctx->d_tables, &ctx->tables_bytes, bytes, false)) != CDH_OK) return rc;
+    double* hd = (double*)ctx->h_tables;
+    for (int h = 0; h < n_hist; ++h) hd[h] = n_pairs[h] / volume;
+    CDH_CUDA(cudaMemcpyAsync(ctx->d_tables, hd, bytes, cudaMemcpyHostToDevice, stream));
+    CDH_CUDA(cudaEventRecord(ctx->staged, stream));
+    ctx->staged_pending = true;
+    RdfParams rp;
+    rp.hist = (const unsigned long long*)hist; rp.density = (const double*)ctx->d_tables; rp.g = g;
+    rp.dr = r_max / (double)n_bins; rp.n_frames = (double)n_frames; rp.n_bins = (uint32_t)n_bins;
+    rp.total = (uint64_t)n_hist * (uint64_t)n_bins;
+    const uint64_t blocks = (rp.total + 255) / 256;
+    if (blocks > 0x7fffffffull) return CDH_ERR_INVALID_ARG;
+    rdf_kernel<<<(unsigned)blocks, 256, 0, stream>>>(rp);
+    CDH_CUDA(cudaGetLastError());
     return CDH_OK;
 }
