@@ -87,7 +87,7 @@ int cdh_create(cdh_ctx **ctx, int device, uint32_t flags);
  *                  CDH_BOX_ORTHO reads the diagonal and requires the off-diagonals to be exactly 0.
  *                  Must be finite and non-singular.
  *  n_boxes         1 (one box for all frames) or n_frames; ignored for CDH_BOX_NONE.
- *  r_max           > 0, finite.  Pairs with !(r < (float)r_max) are dropped in every box mode.
+ *  r_max           > 0, finite (CDH_F64: r_max > 1e-100 and n_bins / r_max < 1e100).  Pairs with !(r < (float)r_max) are dropped in every box mode.
  *  n_bins          1 .. 2^22.  Bin width r_max / n_bins; bin = floor(r * (float)(n_bins / r_max)),
  *                  a kept pair whose product rounds up to n_bins goes to bin n_bins - 1.
  *  precision       CDH_F32 or CDH_F64 (constants are then used in double: r_max, n_bins / r_max, the box).

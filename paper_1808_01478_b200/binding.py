@@ -29,7 +29,7 @@ FLAG_MAX_SMEM_BINS_SHIFT = 8
 
 EXPORTS = ["cdh_create", "cdh_histograms", "cdh_histograms_host", "cdh_destroy", "cdh_strerror",
            "cdh_last_error", "cdh_last_call_info", "cdh_call_kernel_ms", "cdh_rdf",
-           "cdh_bench_fp32_rate", "cdh_bench_shared_atomics", "cdh_selftest_sqrt"]
+           "cdh_bench_fp32_rate", "cdh_bench_shared_atomics", "cdh_selftest_sqrt", "cdh_selftest_sqrt_f64"]
 
 
 class CdhError(RuntimeError):
@@ -79,6 +79,8 @@ def load(path: Optional[str] = None) -> ctypes.CDLL:
                                              ctypes.POINTER(dbl), ctypes.POINTER(dbl), ctypes.POINTER(dbl)]
     lib.cdh_selftest_sqrt.restype = ctypes.c_int
     lib.cdh_selftest_sqrt.argtypes = [u32, u32, vp, ctypes.POINTER(ctypes.c_uint64)]
+    lib.cdh_selftest_sqrt_f64.restype = ctypes.c_int
+    lib.cdh_selftest_sqrt_f64.argtypes = [ctypes.c_uint64, ctypes.c_uint64, vp, ctypes.POINTER(ctypes.c_uint64)]
     if path is None:
         _lib = lib
     return lib
@@ -243,6 +245,15 @@ def cdh_selftest_sqrt(first_bits: int = 0x0D000000, last_bits: int = 0x7F7FFFFF,
     lib = load()
     bad = ctypes.c_uint64()
     rc = lib.cdh_selftest_sqrt(int(first_bits), int(last_bits), _stream_ptr(stream), ctypes.byref(bad))
+    if rc != OK:
+        raise CdhError(rc, cdh_strerror(rc))
+    return int(bad.value)
+
+
+def cdh_selftest_sqrt_f64(seed: int = 1808, count: int = 1 << 32, stream=None) -> int:
+    lib = load()
+    bad = ctypes.c_uint64()
+    rc = lib.cdh_selftest_sqrt_f64(int(seed), int(count), _stream_ptr(stream), ctypes.byref(bad))
     if rc != OK:
         raise CdhError(rc, cdh_strerror(rc))
     return int(bad.value)

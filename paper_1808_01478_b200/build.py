@@ -14,8 +14,16 @@ _HERE = os.path.dirname(os.path.abspath(__file__))
 CSRC = os.path.join(_HERE, "csrc")
 LIB = os.path.join(_HERE, "libcdh.so")
 SOURCES = ["cdh_api.cu", "cdh_bench.cu"]
-DEPS = SOURCES + ["cdh_device.cuh", "cdh_kernels.cuh", "cdh_fast.cuh", "cdh_tile.cuh", "cdh_host.h",
-                  os.path.join("..", "..", "include", "cdh.h"), os.path.join("..", "..", "include", "cdh_bench.h")]
+INCLUDE = os.path.join(_HERE, "..", "include")
+
+
+def deps():
+    """Every source and header the library is built from (all of csrc/ and include/)."""
+    out = [os.path.join(CSRC, f) for f in sorted(os.listdir(CSRC)) if f.endswith((".cu", ".cuh", ".h"))]
+    out += [os.path.join(INCLUDE, f) for f in sorted(os.listdir(INCLUDE)) if f.endswith(".h")]
+    return out
+
+
 NVCC_FLAGS = ["-gencode", "arch=compute_100a,code=sm_100a", "-O3", "-lineinfo", "-std=c++17",
               "-Xcompiler", "-fPIC,-ffp-contract=off,-fno-fast-math", "-shared", "-cudart", "static"]
 
@@ -31,7 +39,7 @@ def is_stale() -> bool:
     if not os.path.exists(LIB):
         return True
     t = os.path.getmtime(LIB)
-    return any(os.path.getmtime(os.path.join(CSRC, d)) > t for d in DEPS)
+    return any(os.path.getmtime(d) > t for d in deps())
 
 
 def build(force: bool = False, verbose: bool = False, extra_flags=(), out: str = LIB) -> str:

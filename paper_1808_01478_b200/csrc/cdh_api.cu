@@ -350,6 +350,8 @@ extern "C" int cdh_histograms(cdh_ctx* ctx, const void* coords, int32_t n_frames
     if (rc != CDH_OK) return rc;
     cudaStream_t stream = (cudaStream_t)stream_;
     ctx->err.clear();
+    // the double-precision kernels bin sqrt(d2) < 2^-485 as 0: harmless while it lands in bin 0 and is kept
+    if (precision == CDH_F64 && !(r_max > 1e-100 && (double)n_bins / r_max < 1e100)) return CDH_ERR_INVALID_ARG;
     if (precision == CDH_F64)
         return histograms_f64(ctx, (const double*)coords, n_frames, off, n_species, box_type, box, n_boxes, r_max, n_bins, stream, out);
 

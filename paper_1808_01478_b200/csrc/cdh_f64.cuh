@@ -10,6 +10,7 @@
 // buffer; a j-stage is 512 particles = 12 KB, two stages filled by 1-D TMA bulk copies.
 #pragma once
 #include "cdh_tile.cuh"
+#include "cdh_sqrt64.cuh"
 
 namespace cdh {
 
@@ -106,15 +107,17 @@ constexpr double kPruneLimit64 = 0.5 - 9.313225746154785e-10;     // 1/2 - 2^-30
 constexpr float kPruneRange64 = 1024.0f;                          // fractional range up to which pruning is proven
 
 // d2 of one pair.  prune: the zero-shift candidate may be accepted when every |s_k - n_k| <= 1/2 - 2^-30.
+struct OrthoRegs64 { double L[3], invL[3]; };      // the orthorhombic constants, held in registers
+
 template <int BOX>
 __device__ __forceinline__ double pair_d2_f64(double xi, double yi, double zi, double xj, double yj, double zj,
-                                              const BoxConst64* __restrict__ bc, bool prune) {
+                                              const BoxConst64* __restrict__ bc, const OrthoRegs64& ob, bool prune) {
     double dx = __dsub_rn(xj, xi), dy = __dsub_rn(yj, yi), dz = __dsub_rn(zj, zi);
     if constexpr (BOX == BOX_ORTHO) {
         double n;
-        n = rint(__dmul_rn(dx, bc->invL[0])); dx = __dsub_rn(dx, __dmul_rn(bc->L[0], n));
-        n = rint(__dmul_rn(dy, bc->invL[1])); dy = __dsub_rn(dy, __dmul_rn(bc->L[1], n));
-        n = rint(__dmul_rn(dz, bc->invL[2])); dz = __dsub_rn(dz, __dmul_rn(bc->L[2], n));
+        n = rint(__dmul_rn(dx, ob.invL[0])); dx = __dsub_rn(dx, __dmul_rn(ob.L[0], n));
+        n = rint(__dmul_rn(dy, ob.invL[1])); dy = __dsub_rn(dy, __dmul_rn(ob.L[1], n));
+        n = rint(__dmul_rn(dz, ob.invL[2])); dz = __dsub_rn(dz, __dmul_rn(ob.L[2], n));
     } else if constexpr (BOX == BOX_TRI) {
         double n[3], e[3], fm = 0.0;
         const double d[3] = {dx, dy, dz};
@@ -147,12 +150,11 @@ __device__ __forceinline__ double pair_d2_f64(double xi, double yi, double zi, d
 
 __device__ __forceinline__ void bin_f64(double d2, double rmax, double scale, uint32_t n_bins, uint32_t hist,
                                         uint32_t bin_lo, uint32_t lim, uint32_t trash, bool keep) {
-    const double d = __dsqrt_rn(d2);
-    keep = keep && (d < rmax);                            // drops d >= r_max and NaN
-    const double t = floor(__dmul_rn(d, scale));
-    uint32_t b = keep ? (uint32_t)fmin(t, 4294967040.0) : 0u;
-    b = min(b, n_bins - 1u) - bin_lo;                     // reading Q3; unsigned wrap for bins below the sweep
-    hist_inc((keep && b < lim) ? hist + 4u * b : trash);
+    bool finite;
+    const double d = sqrt_rn_f64(d2, finite);
+    const uint32_t f = __double2uint_rd(__dmul_rn(d, scale));   // floor, saturating (one F2I)
+    const uint32_t b = min(f, n_bins - 1u) - bin_lo;            // reading Q3; unsigned wrap for bins below the sweep
+    hist_inc((keep && finite && (d < rmax) && b < lim) ? hist + 4u * b : trash);
 }
 
 // ---- K1 for doubles: same schedule, stages and flush rule as tile_kernel (cdh_tile.cuh) ------------
@@ -237,6 +239,11 @@ __global__ void __launch_bounds__(T, MINB) tile_kernel_f64(const TileParams64 P)
         const uint32_t s_begin = (masked && i0 > j0) ? (i0 - j0) / kStageParticles : 0;
         const double* jsrc = P.pk + ((size_t)seg.j_group + (j0 >> 2)) * kGroupFloats;
         const bool prune = (BOX == BOX_TRI) ? (range_ok && s_box->prune_ok != 0.0) : true;
+        OrthoRegs64 ob;
+        if constexpr (BOX == BOX_ORTHO) {
+#pragma unroll
+            for (int k = 0; k < 3; ++k) { ob.L[k] = s_box->L[k]; ob.invL[k] = s_box->invL[k]; }
+        }
 
         if (tid == 0 && s_begin < n_stage) {
             const uint32_t b = stage_cnt & 1u;
@@ -267,7 +274,7 @@ __global__ void __launch_bounds__(T, MINB) tile_kernel_f64(const TileParams64 P)
 #pragma unroll
                         for (int r = 0; r < kR; ++r) {
                             const bool keep = !stage_masked || (jg + 2 * h + c > ig + r);
-                            const double d2 = pair_d2_f64<BOX>(xi[r], yi[r], zi[r], xj[c], yj[c], zj[c], s_box, prune);
+                            const double d2 = pair_d2_f64<BOX>(xi[r], yi[r], zi[r], xj[c], yj[c], zj[c], s_box, ob, prune);
                             bin_f64(d2, P.rmax, P.scale, P.n_bins, hist_addr, cur_lo, cur_lim, trash_addr, keep);
                         }
                 }

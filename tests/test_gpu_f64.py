@@ -103,3 +103,9 @@ def test_f64_config2_full_size():
     got, info = gpu64(p)
     same(got, oracle64(p), f"config 2 full size in double {info}")
     assert got.sum() / p.evaluated_pairs == pytest.approx(math.pi / 6, rel=2e-3)
+
+
+def test_f64_sqrt_selftest_sample():
+    if not torch.cuda.is_available():
+        pytest.skip("no CUDA device")
+    assert cdh.cdh_selftest_sqrt_f64(7, 1 << 28) == 0
