@@ -235,9 +235,11 @@ static int histograms_f64(cdh_ctx* ctx, const double* coords, int32_t n_frames, 
     const int smem_bytes = tile_smem_bytes64((int)sp.bins_per_sweep);
     const bool big = 2 * (smem_bytes + 1024) > 228 * 1024;
     TileFn64 fn; int threads;
-    if (box_type == CDH_BOX_NONE) { fn = big ? tile_kernel_f64<BOX_NONE, 512, 1> : tile_kernel_f64<BOX_NONE, 256, 2>; }
-    else if (box_type == CDH_BOX_ORTHO) { fn = big ? tile_kernel_f64<BOX_ORTHO, 512, 1> : tile_kernel_f64<BOX_ORTHO, 256, 2>; }
-    else { fn = big ? tile_kernel_f64<BOX_TRI, 512, 1> : tile_kernel_f64<BOX_TRI, 256, 2>; }
+    const bool pbox = box_type == CDH_BOX_TRICLINIC && nb == 1;      // one box: constants through the parameter bank
+    if (box_type == CDH_BOX_NONE) { fn = big ? tile_kernel_f64<BOX_NONE, 512, 1, false> : tile_kernel_f64<BOX_NONE, 256, 2, false>; }
+    else if (box_type == CDH_BOX_ORTHO) { fn = big ? tile_kernel_f64<BOX_ORTHO, 512, 1, false> : tile_kernel_f64<BOX_ORTHO, 256, 2, false>; }
+    else if (pbox) { fn = big ? tile_kernel_f64<BOX_TRI, 512, 1, true> : tile_kernel_f64<BOX_TRI, 256, 2, true>; }
+    else { fn = big ? tile_kernel_f64<BOX_TRI, 512, 1, false> : tile_kernel_f64<BOX_TRI, 256, 2, false>; }
     threads = big ? 512 : 256;
     const uint32_t ti = (uint32_t)threads * kR;
     CDH_CUDA(cudaFuncSetAttribute((const void*)fn, cudaFuncAttributeMaxDynamicSharedMemorySize, smem_bytes));
@@ -307,6 +309,7 @@ static int histograms_f64(cdh_ctx* ctx, const double* coords, int32_t n_frames, 
         tp.n_rows = (uint32_t)wt.rows.size() - 1; tp.n_items = (uint32_t)wt.n_items;
         tp.n_bins = (uint32_t)n_bins; tp.tj = tj; tp.smem_bins = sp.bins_per_sweep;
         tp.rmax = r_max; tp.scale = (double)n_bins / r_max;
+        tp.box0 = boxes[0];
         grid = grid_full < tp.n_items ? grid_full : tp.n_items;
         fn<<<grid, threads, smem_bytes, stream>>>(tp);
         CDH_CUDA(cudaGetLastError());

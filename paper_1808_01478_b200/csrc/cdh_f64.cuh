@@ -37,6 +37,8 @@ struct TileParams64 {
     uint32_t tj;
     uint32_t smem_bins;
     double rmax, scale;         // r_max, n_bins / r_max
+    BoxConst64 box0;            // PBOX variants (one box for all frames): the constants sit in the kernel-parameter
+                                // constant bank and are used as c[0x0][..] operands, no shared-memory loads
 };
 
 __host__ __device__ constexpr int tile_smem_bytes64(int smem_bins) {
@@ -111,7 +113,8 @@ struct OrthoRegs64 { double L[3], invL[3]; };      // the orthorhombic constants
 
 template <int BOX>
 __device__ __forceinline__ double pair_d2_f64(double xi, double yi, double zi, double xj, double yj, double zj,
-                                              const BoxConst64* __restrict__ bc, const OrthoRegs64& ob, bool prune) {
+                                              const BoxConst64& bcr, const OrthoRegs64& ob, bool prune) {
+    const BoxConst64* __restrict__ bc = &bcr;
     double dx = __dsub_rn(xj, xi), dy = __dsub_rn(yj, yi), dz = __dsub_rn(zj, zi);
     if constexpr (BOX == BOX_ORTHO) {
         double n;
@@ -158,7 +161,7 @@ __device__ __forceinline__ void bin_f64(double d2, double rmax, double scale, ui
 }
 
 // ---- K1 for doubles: same schedule, stages and flush rule as tile_kernel (cdh_tile.cuh) ------------
-template <int BOX, int T, int MINB>
+template <int BOX, int T, int MINB, bool PBOX>
 __global__ void __launch_bounds__(T, MINB) tile_kernel_f64(const TileParams64 P) {
     extern __shared__ __align__(128) unsigned char smem[];
     constexpr int TI = T * kR;
@@ -274,7 +277,9 @@ __global__ void __launch_bounds__(T, MINB) tile_kernel_f64(const TileParams64 P)
 #pragma unroll
                         for (int r = 0; r < kR; ++r) {
                             const bool keep = !stage_masked || (jg + 2 * h + c > ig + r);
-                            const double d2 = pair_d2_f64<BOX>(xi[r], yi[r], zi[r], xj[c], yj[c], zj[c], s_box, ob, prune);
+                            double d2;
+                            if constexpr (PBOX) d2 = pair_d2_f64<BOX>(xi[r], yi[r], zi[r], xj[c], yj[c], zj[c], P.box0, ob, prune);
+                            else d2 = pair_d2_f64<BOX>(xi[r], yi[r], zi[r], xj[c], yj[c], zj[c], *s_box, ob, prune);
                             bin_f64(d2, P.rmax, P.scale, P.n_bins, hist_addr, cur_lo, cur_lim, trash_addr, keep);
                         }
                 }
