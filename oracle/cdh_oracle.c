@@ -37,7 +37,8 @@
  * Parity pins (tests/test_oracle_pins.py, -m "not gpu"): total counts N(N-1)/2 and N1*N2, the
  * hand-computed 4-particle examples in tests/golden/, 125-image brute force on tiny dyadic
  * periodic boxes, permutation / species-swap symmetry, numpy reduction in the non-periodic case,
- * ideal-gas shell counts, the > 2^32 single-bin case.
+ * ideal-gas shell counts, the > 2^32 single-bin case; for cdh_oracle_rdf (tests/test_oracle_rdf.py): the ideal gas
+ * g = 1, a simple-cubic crystal's peaks and coordination numbers, the bin-centre shell identity, scaling laws.
  *
  * Threads: OpenMP over the outer particle loop with thread-private uint64 histograms summed at the
  * end (integer sums are order free).  This is for wall time only.
