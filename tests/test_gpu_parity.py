@@ -288,3 +288,47 @@ def test_user_stream_and_back_to_back_calls():
         s.synchronize()
         for o in outs:
             assert_same(o.cpu().numpy().view(np.uint64), oracle_hist(p), "stream")
+
+
+def test_many_species_and_ragged_sizes():
+    # 12 species of very different sizes (some empty, some of one particle): 78 histograms in one call
+    counts = (0, 1, 2, 3, 511, 512, 513, 1023, 1025, 0, 2047, 4097)
+    p = inputs.uniform_problem(21, counts, inputs.BOX_ORTHO, 777, 2.0, box=np.diag([4.0, 5.0, 6.0]))
+    got, info = gpu_hist(p)
+    assert got.shape == (78, 777)
+    assert_same(got, oracle_hist(p), f"12 species {info}")
+
+
+def test_per_frame_triclinic_boxes_and_frame_sum():
+    g = np.random.Generator(np.random.PCG64(33))
+    f, n = 4, 1500
+    boxes = np.stack([np.array([[7.0 + k, 0, 0], [1.0, 6.5, 0], [0.5 * k, -1.0, 8.0 - k]]) for k in range(f)])
+    coords = np.stack([(g.random((n, 3)) @ boxes[k]).astype(np.float32) for k in range(f)])
+    p = inputs.Problem("tri_per_frame", coords, np.array([0, 400, n], dtype=np.int32), inputs.BOX_TRICLINIC,
+                       boxes.reshape(f, 9), 2.4, 999)
+    got, _ = gpu_hist(p)
+    assert_same(got, oracle_hist(p), p.name)
+    # Eq. 2: the call sums the frames
+    parts = sum(gpu_hist(inputs.Problem(f"fr{k}", coords[k:k + 1], p.species_offsets, p.box_type, p.box[k:k + 1], p.r_max,
+                                        p.n_bins))[0] for k in range(f))
+    assert_same(got, parts, "sum over frames")
+
+
+def test_maximum_bin_count_and_single_bin():
+    p = inputs.uniform_problem(5, (3000,), inputs.BOX_NONE, 1 << 22, math.sqrt(3.0))      # n_bins = 2^22, the API maximum
+    got, info = gpu_hist(p)
+    assert info["global_hist"]
+    assert_same(got, oracle_hist(p), f"2^22 bins {info}")
+    q = inputs.uniform_problem(6, (3000, 10), inputs.BOX_NONE, 1, 0.5)
+    got, _ = gpu_hist(q)
+    assert_same(got, oracle_hist(q), "one bin")
+
+
+def test_tiny_rmax_keeps_nothing_and_huge_rmax_keeps_everything():
+    p = inputs.uniform_problem(8, (2500,), inputs.BOX_NONE, 100, 1e-6)
+    got, _ = gpu_hist(p)
+    assert_same(got, oracle_hist(p), "r_max = 1e-6")
+    q = inputs.uniform_problem(8, (2500,), inputs.BOX_NONE, 100, 1e6)
+    got, _ = gpu_hist(q)
+    assert int(got.sum()) == 2500 * 2499 // 2 and int(got[0, 0]) == int(got.sum())
+    assert_same(got, oracle_hist(q), "r_max = 1e6")
