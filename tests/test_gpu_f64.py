@@ -109,3 +109,43 @@ def test_f64_sqrt_selftest_sample():
     if not torch.cuda.is_available():
         pytest.skip("no CUDA device")
     assert cdh.cdh_selftest_sqrt_f64(7, 1 << 28) == 0
+
+
+@pytest.mark.parametrize("seed", [21, 22, 23])
+def test_f64_ortho_fused_and_plain_rint_awkward_boxes(seed):
+    g = np.random.Generator(np.random.PCG64(seed))
+    L = g.uniform(3.0, 40.0, size=3) * np.array([1.0, 1.0 / 3.0, math.pi])
+    p = inputs.uniform_problem(seed, (1200, 1700), inputs.BOX_ORTHO, 5000, 0.5 * float(L.min()), box=np.diag(L))
+    want = oracle64(p)
+    a, _ = gpu64(p)                              # fused rint (coordinates inside the box)
+    b, _ = gpu64(p, cdh.FLAG_NO_PRUNE)           # plain rint
+    same(a, want, f"f64 fused rint L={L}")
+    same(b, want, "f64 plain rint")
+    q = inputs.uniform_problem(seed, (900, 800), inputs.BOX_ORTHO, 3000, 0.5 * float(L.min()), box=np.diag(L), spread=4.0)
+    c, _ = gpu64(q)                              # range 4 > 1.49: the kernel itself falls back to the plain form
+    same(c, oracle64(q), "f64 unwrapped coordinates")
+
+
+def test_f64_ortho_half_box_switch_points():
+    L = np.array([10.0, 7.3, 12.9])
+    rows = [[0.0, 0.0, 0.0]]
+    for ax in range(3):
+        half = np.float64(L[ax] / 2)
+        for k in range(-6, 7):
+            v = half
+            for _ in range(abs(k)):
+                v = np.nextafter(v, np.inf if k > 0 else -np.inf)
+            q = [0.0, 0.0, 0.0]; q[ax] = float(v)
+            rows.append(q)
+    pts = np.array(rows, dtype=np.float64)[None]
+    off = np.array([0, 1, len(rows)], dtype=np.int32)
+    box = np.diag(L).reshape(1, 9)
+    want = cdh_oracle.histograms(pts, off, inputs.BOX_ORTHO, box, 30.0, 1 << 20, precision="f64")
+    if not torch.cuda.is_available():
+        pytest.skip("no CUDA device")
+    with cdh.Context(0) as ctx:
+        d = torch.from_numpy(pts).cuda()
+        out = torch.empty((3, 1 << 20), dtype=torch.int64, device="cuda")
+        ctx.cdh_histograms(d, 1, off, inputs.BOX_ORTHO, box, 30.0, 1 << 20, out, precision=cdh.F64)
+        torch.cuda.synchronize()
+    same(out.cpu().numpy().view(np.uint64), want, "f64 pairs within 6 ulp of L/2")
