@@ -236,10 +236,15 @@ static int histograms_f64(cdh_ctx* ctx, const double* coords, int32_t n_frames, 
     const bool big = 2 * (smem_bytes + 1024) > 228 * 1024;
     TileFn64 fn; int threads;
     const bool pbox = box_type == CDH_BOX_TRICLINIC && nb == 1;      // one box: constants through the parameter bank
-    if (box_type == CDH_BOX_NONE) { fn = big ? tile_kernel_f64<BOX_NONE, 512, 1, false> : tile_kernel_f64<BOX_NONE, 256, 2, false>; }
-    else if (box_type == CDH_BOX_ORTHO) { fn = big ? tile_kernel_f64<BOX_ORTHO, 512, 1, false> : tile_kernel_f64<BOX_ORTHO, 256, 2, false>; }
-    else if (pbox) { fn = big ? tile_kernel_f64<BOX_TRI, 512, 1, true> : tile_kernel_f64<BOX_TRI, 256, 2, true>; }
-    else { fn = big ? tile_kernel_f64<BOX_TRI, 512, 1, false> : tile_kernel_f64<BOX_TRI, 256, 2, false>; }
+    const bool split64 = sp.n_sweeps > 1;
+    auto pick64 = [&](auto split_c) -> TileFn64 {
+        constexpr bool S = decltype(split_c)::value;
+        if (box_type == CDH_BOX_NONE) return big ? tile_kernel_f64<BOX_NONE, 512, 1, false, S> : tile_kernel_f64<BOX_NONE, 256, 2, false, S>;
+        if (box_type == CDH_BOX_ORTHO) return big ? tile_kernel_f64<BOX_ORTHO, 512, 1, false, S> : tile_kernel_f64<BOX_ORTHO, 256, 2, false, S>;
+        if (pbox) return big ? tile_kernel_f64<BOX_TRI, 512, 1, true, S> : tile_kernel_f64<BOX_TRI, 256, 2, true, S>;
+        return big ? tile_kernel_f64<BOX_TRI, 512, 1, false, S> : tile_kernel_f64<BOX_TRI, 256, 2, false, S>;
+    };
+    fn = split64 ? pick64(std::true_type{}) : pick64(std::false_type{});
     threads = big ? 512 : 256;
     const uint32_t ti = (uint32_t)threads * kR;
     CDH_CUDA(cudaFuncSetAttribute((const void*)fn, cudaFuncAttributeMaxDynamicSharedMemorySize, smem_bytes));

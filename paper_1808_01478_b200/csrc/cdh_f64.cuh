@@ -151,17 +151,19 @@ __device__ __forceinline__ double pair_d2_f64(double xi, double yi, double zi, d
     return __dadd_rn(__dadd_rn(__dmul_rn(dx, dx), __dmul_rn(dy, dy)), __dmul_rn(dz, dz));
 }
 
-__device__ __forceinline__ void bin_f64(double d2, double rmax, double scale, uint32_t n_bins, uint32_t hist,
+template <bool SPLIT>
+__device__ __forceinline__ void bin_f64(double d2, double rmax, double scale, uint32_t last_bin, uint32_t hist,
                                         uint32_t bin_lo, uint32_t lim, uint32_t trash, bool keep) {
-    bool finite;
-    const double d = sqrt_rn_f64(d2, finite);
+    const double d = sqrt_rn_f64(d2);
     const uint32_t f = __double2uint_rd(__dmul_rn(d, scale));   // floor, saturating (one F2I)
-    const uint32_t b = min(f, n_bins - 1u) - bin_lo;            // reading Q3; unsigned wrap for bins below the sweep
-    hist_inc((keep && finite && (d < rmax) && b < lim) ? hist + 4u * b : trash);
+    const uint32_t b = min(f, last_bin) - bin_lo;               // reading Q3; unsigned wrap for bins below the sweep
+    bool ok = keep && (d < rmax);                               // false for NaN (NaN input, +inf)
+    if constexpr (SPLIT) ok = ok && b < lim;
+    hist_inc(ok ? hist + 4u * b : trash);
 }
 
 // ---- K1 for doubles: same schedule, stages and flush rule as tile_kernel (cdh_tile.cuh) ------------
-template <int BOX, int T, int MINB, bool PBOX>
+template <int BOX, int T, int MINB, bool PBOX, bool SPLIT>
 __global__ void __launch_bounds__(T, MINB) tile_kernel_f64(const TileParams64 P) {
     extern __shared__ __align__(128) unsigned char smem[];
     constexpr int TI = T * kR;
@@ -265,25 +267,29 @@ __global__ void __launch_bounds__(T, MINB) tile_kernel_f64(const TileParams64 P)
             const uint32_t jbase = j0 + s * kStageParticles;
             const uint32_t n_grp = (min(j1 - jbase, (uint32_t)kStageParticles) + 3u) >> 2;
             const bool stage_masked = masked && (jbase < i0 + TI);
+            auto body = [&](auto masked_c) {
+                constexpr bool MASKED = decltype(masked_c)::value;
 #pragma unroll 1
-            for (uint32_t g = 0; g < n_grp; ++g) {
-                const uint32_t jg = jbase + 4u * g;
+                for (uint32_t g = 0; g < n_grp; ++g) {
+                    const uint32_t jg = jbase + 4u * g;
 #pragma unroll
-                for (int h = 0; h < 2; ++h) {                   // two j-particles at a time (register pressure)
-                    const double2 XJ = sj[6 * g + h], YJ = sj[6 * g + 2 + h], ZJ = sj[6 * g + 4 + h];
-                    const double xj[2] = {XJ.x, XJ.y}, yj[2] = {YJ.x, YJ.y}, zj[2] = {ZJ.x, ZJ.y};
+                    for (int h = 0; h < 2; ++h) {                   // two j-particles at a time (register pressure)
+                        const double2 XJ = sj[6 * g + h], YJ = sj[6 * g + 2 + h], ZJ = sj[6 * g + 4 + h];
+                        const double xj[2] = {XJ.x, XJ.y}, yj[2] = {YJ.x, YJ.y}, zj[2] = {ZJ.x, ZJ.y};
 #pragma unroll
-                    for (int c = 0; c < 2; ++c)
+                        for (int c = 0; c < 2; ++c)
 #pragma unroll
-                        for (int r = 0; r < kR; ++r) {
-                            const bool keep = !stage_masked || (jg + 2 * h + c > ig + r);
-                            double d2;
-                            if constexpr (PBOX) d2 = pair_d2_f64<BOX>(xi[r], yi[r], zi[r], xj[c], yj[c], zj[c], P.box0, ob, prune);
-                            else d2 = pair_d2_f64<BOX>(xi[r], yi[r], zi[r], xj[c], yj[c], zj[c], *s_box, ob, prune);
-                            bin_f64(d2, P.rmax, P.scale, P.n_bins, hist_addr, cur_lo, cur_lim, trash_addr, keep);
-                        }
+                            for (int r = 0; r < kR; ++r) {
+                                const bool keep = !MASKED || (jg + 2 * h + c > ig + r);
+                                double d2;
+                                if constexpr (PBOX) d2 = pair_d2_f64<BOX>(xi[r], yi[r], zi[r], xj[c], yj[c], zj[c], P.box0, ob, prune);
+                                else d2 = pair_d2_f64<BOX>(xi[r], yi[r], zi[r], xj[c], yj[c], zj[c], *s_box, ob, prune);
+                                bin_f64<SPLIT>(d2, P.rmax, P.scale, P.n_bins - 1u, hist_addr, cur_lo, cur_lim, trash_addr, keep);
+                            }
+                    }
                 }
-            }
+            };
+            if (stage_masked) body(std::true_type{}); else body(std::false_type{});
             __syncthreads();
             ++stage_cnt;
         }
