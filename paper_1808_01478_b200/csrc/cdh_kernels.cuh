@@ -60,13 +60,20 @@ __device__ __forceinline__ uint32_t float_key(float v) {
 __device__ __forceinline__ float key_float(uint32_t k) {
     return __uint_as_float((k & 0x80000000u) ? (k & 0x7fffffffu) : ~k);
 }
-// Largest extent over the three axes of the fractional coordinates of all particles of the call (0 if none).
+// Largest extent over the three axes of the fractional coordinates of all particles of the call (0 if none), made
+// conservative for coordinates far from the origin: the keys come from fp32 evaluations of b^-1 x whose absolute
+// error grows with |b^-1 x|, so the result is max(max - min, max|b^-1 x| * 1.49 / 4096): the 1.49 limit of the fused
+// rint / exact-B*n paths then also implies |b^-1 x| <= 4096 (range error < 1e-3, far inside the 0.01 margin to 3/2),
+// and the 2^20 limit of the magic-number rint implies |b^-1 x| < 2^32.
 __device__ __forceinline__ float frac_range(const unsigned int* __restrict__ keys) {
     float r = 0.0f;
 #pragma unroll
     for (int q = 0; q < 3; ++q) {
         const uint32_t kmax = __ldg(keys + q), kmin_c = __ldg(keys + 3 + q);
-        if (kmax != 0u) r = fmaxf(r, key_float(kmax) - key_float(~kmin_c));
+        if (kmax != 0u) {
+            const float hi = key_float(kmax), lo = key_float(~kmin_c);
+            r = fmaxf(r, fmaxf(hi - lo, fmaxf(fabsf(hi), fabsf(lo)) * (1.49f / 4096.0f)));
+        }
     }
     return r;
 }

@@ -332,3 +332,17 @@ def test_tiny_rmax_keeps_nothing_and_huge_rmax_keeps_everything():
     got, _ = gpu_hist(q)
     assert int(got.sum()) == 2500 * 2499 // 2 and int(got[0, 0]) == int(got.sum())
     assert_same(got, oracle_hist(q), "r_max = 1e6")
+
+
+def test_periodic_boxes_far_from_the_origin():
+    # compact systems translated far away: fp32 coordinates get coarse (ulp(x) up to a fraction of the bin width) and the
+    # measured fractional range loses accuracy; the launch plan must leave the fused / pruned paths early enough
+    base = inputs.uniform_problem(41, (900, 1100), inputs.BOX_ORTHO, 2000, 3.0, box=np.diag([6.0, 7.3, 9.1]))
+    tri_box = np.array([[7.0, 0.0, 0.0], [1.0, 6.5, 0.0], [0.5, -1.0, 8.0]])
+    tri = inputs.uniform_problem(42, (800, 1000), inputs.BOX_TRICLINIC, 2000, 3.0, box=tri_box)
+    for shift in (1.0e2, 3.0e3, 1.0e4, 3.0e5, 1.0e7):
+        for p in (base, tri):
+            q = inputs.Problem(f"far{shift}", (p.coords.astype(np.float64) + shift).astype(np.float32), p.species_offsets,
+                               p.box_type, p.box, p.r_max, p.n_bins)
+            got, info = gpu_hist(q)
+            assert_same(got, oracle_hist(q), f"box_type {p.box_type} shifted by {shift} {info}")
