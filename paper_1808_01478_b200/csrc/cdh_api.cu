@@ -70,6 +70,10 @@ struct Variant { TileFn fn; int threads; };
                               // break-even: 200,000 uniform points, 400,000 bins: 8 sweeps 200 vs global 221 Gpairs/s)
 #endif
 constexpr uint32_t kGlobalSweeps = CDH_GLOBAL_SWEEPS;
+#ifndef CDH_ITEMS_PER_CTA
+#define CDH_ITEMS_PER_CTA 64   // work items per resident CTA the j-chunk size is shrunk for (tail of the dynamic schedule)
+#endif
+constexpr uint64_t kItemsPerCta = CDH_ITEMS_PER_CTA;
 #ifndef CDH_MINB
 #define CDH_MINB 3      // resident CTAs per SM the 256-thread NONE / ORTHO fast variants are register-bounded for
                         // (80 registers; measured +1.5 % over 2; the triclinic variants need 128 registers: 2)
@@ -257,7 +261,7 @@ static int histograms_f64(cdh_ctx* ctx, const double* coords, int32_t n_frames, 
     uint32_t tj = 8192;
     for (;; tj >>= 1) {
         build_tables(n_frames, off, n_species, nb > 0 ? nb : 1, (uint32_t)n_bins, sp, ti, tj, pad_off, frame_slots, &wt);
-        if (wt.n_items >= 16ull * grid_full || tj == (uint32_t)kStageParticles) break;
+        if (wt.n_items >= kItemsPerCta * grid_full || tj == (uint32_t)kStageParticles) break;
     }
     if (wt.n_items >= 0xffffffffull || wt.rows.size() >= 0x7fffffffull) return CDH_ERR_INVALID_ARG;
 
@@ -443,7 +447,7 @@ extern "C" int cdh_histograms(cdh_ctx* ctx, const void* coords, int32_t n_frames
     uint32_t tj = 8192;
     for (;; tj >>= 1) {
         build_tables(n_frames, off, n_species, nb > 0 ? nb : 1, (uint32_t)n_bins, sp, ti, tj, pad_off, frame_slots, &wt);
-        if (wt.n_items >= 16ull * grid_full || tj == (uint32_t)kStageParticles) break;
+        if (wt.n_items >= kItemsPerCta * grid_full || tj == (uint32_t)kStageParticles) break;
     }
     if (wt.n_items >= 0xffffffffull || wt.rows.size() >= 0x7fffffffull) return CDH_ERR_INVALID_ARG;
 
