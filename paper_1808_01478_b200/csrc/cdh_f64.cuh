@@ -7,7 +7,7 @@
 // DESIGN.md "Triclinic pruning"; the margins are far wider in double).
 //
 // Layout: groups of 4 particles, 12 doubles per group  x0..3 | y0..3 | z0..3  (96 bytes), NaN padded like the fp32
-// buffer; a j-stage is 512 particles = 12 KB, two stages filled by 1-D TMA bulk copies.
+// buffer; a j-stage is 256 particles = 6 KB, two stages filled by 1-D TMA bulk copies.
 #pragma once
 #include "cdh_tile.cuh"
 #include "cdh_sqrt64.cuh"

@@ -4,7 +4,7 @@
 // and the paper's shared-memory kernel) and pulls work items (i-tile, j-chunk) from a
 // global counter.  Items are ordered by (histogram row, bin sweep), so a CTA flushes into the uint64
 // result only when that key changes, when its increment budget nears 2^32 and at exit.
-// Each thread keeps R = 4 i-particles in registers; the j-chunk streams through two 6 KB shared-memory
+// Each thread keeps R = 4 i-particles in registers; the j-chunk streams through two 3 KB shared-memory
 // stages filled by 1-D TMA bulk copies (cp.async.bulk + mbarrier); all lanes read the same j-group
 // (LDS.128 broadcast).  Intra-species segments only schedule j-chunks that reach above the diagonal
 // (triangular schedule, Fig. 1, 223-225); tiles on the diagonal take the masked path.
