@@ -126,7 +126,8 @@ const char *cdh_last_error(const cdh_ctx *ctx);
  *   info[0] = kernels launched by the call      info[1] = work items (tile pairs) scheduled
  *   info[2] = bin-range sweeps                   info[3] = CTAs of the tile kernel
  *   info[4] = threads per CTA                    info[5] = dynamic shared memory bytes per CTA
- *   info[6] = kernel variant id                  info[7] = evaluated pairs incl. padding lanes (low 32 bits unused; see info64)
+ *   info[6] = kernel variant id (bit 0 fast path, bit 2 global histogram, bits 4-7 box type, bits 8-11 form: ORTHO 0 plain /
+ *             1 fused / 2 exact-product rint, TRICLINIC zero structure; bits 16.. j-chunk size)                  info[7] = evaluated pairs incl. padding lanes (low 32 bits unused; see info64)
  * Returns CDH_OK or CDH_ERR_INVALID_ARG. */
 int cdh_last_call_info(const cdh_ctx *ctx, int64_t info[8]);
 

@@ -91,7 +91,8 @@ template <int SPLIT>
 Variant pick_fast(int box_type, int tri, bool big) {      // tri: TRI_* for TRICLINIC, ORTHO_* for ORTHO
     if (box_type == CDH_BOX_NONE) return fast_variant<BOX_NONE, 0, SPLIT>(big);
     if (box_type == CDH_BOX_ORTHO)
-        return tri == ORTHO_FUSED ? fast_variant<BOX_ORTHO, ORTHO_FUSED, SPLIT>(big) : fast_variant<BOX_ORTHO, ORTHO_PLAIN, SPLIT>(big);
+        return tri == ORTHO_FUSED ? fast_variant<BOX_ORTHO, ORTHO_FUSED, SPLIT>(big)
+             : tri == ORTHO_EXACT ? fast_variant<BOX_ORTHO, ORTHO_EXACT, SPLIT>(big) : fast_variant<BOX_ORTHO, ORTHO_PLAIN, SPLIT>(big);
     if (tri == TRI_UPPER_B01) return fast_variant<BOX_TRI, TRI_UPPER_B01, SPLIT>(big);
     if (tri == TRI_UPPER) return fast_variant<BOX_TRI, TRI_UPPER, SPLIT>(big);
     return fast_variant<BOX_TRI, TRI_GENERAL, SPLIT>(big);
@@ -412,8 +413,8 @@ extern "C" int cdh_histograms(cdh_ctx* ctx, const void* coords, int32_t n_frames
                                  !(scale_f < 5.0e14f);
     // Launch plan: every tile launch of the call owns an interval (lo, hi] of the fractional-coordinate range the
     // repack kernel measures, and exactly one of them does the work (cdh_tile.cuh).
-    //   ORTHO: fused rint up to 1.49 (if the host found its constants for every box), magic-number rint up to
-    //          2^20, library rintf beyond;  TRICLINIC: fast path up to 1.49 (n in {-1,0,1}), definition beyond.
+    //   ORTHO: fused rint up to 1.49 (exact-product form if the host found no fused constants for some box),
+    //          magic-number rint up to 2^20, library rintf beyond;  TRICLINIC: fast path up to 1.49 (n in {-1,0,1}), definition beyond.
     struct Launch { Variant v; float lo, hi; };
     const float kInf = INFINITY, kSmall = 1.49f, kMagic = 1048576.0f;
     bool fused_ok = box_type == CDH_BOX_ORTHO;
@@ -428,8 +429,9 @@ extern "C" int cdh_histograms(cdh_ctx* ctx, const void* coords, int32_t n_frames
     if (use_simple_only) plan.push_back({vs, -kInf, kInf});
     else if (box_type == CDH_BOX_NONE) plan.push_back({fast_of(0), -kInf, kInf});
     else if (box_type == CDH_BOX_ORTHO) {
-        if (fused_ok) { plan.push_back({fast_of(ORTHO_FUSED), -kInf, kSmall}); plan.push_back({fast_of(ORTHO_PLAIN), kSmall, kMagic}); }
-        else plan.push_back({fast_of(ORTHO_PLAIN), -kInf, kMagic});
+        const bool plain_only = (ctx->flags & CDH_FLAG_NO_PRUNE) != 0;     // tests: the pinned 5-operation form everywhere
+        if (plain_only) plan.push_back({fast_of(ORTHO_PLAIN), -kInf, kMagic});
+        else { plan.push_back({fast_of(fused_ok ? ORTHO_FUSED : ORTHO_EXACT), -kInf, kSmall}); plan.push_back({fast_of(ORTHO_PLAIN), kSmall, kMagic}); }
         plan.push_back({vs, kMagic, kInf});
     } else {
         plan.push_back({fast_of(tri), -kInf, kSmall});
@@ -524,7 +526,8 @@ extern "C" int cdh_histograms(cdh_ctx* ctx, const void* coords, int32_t n_frames
     }
     ctx->info[0] = launches; ctx->info[1] = (int64_t)wt.n_items; ctx->info[2] = sp.n_sweeps; ctx->info[3] = grid;
     ctx->info[4] = vf.threads; ctx->info[5] = smem_bytes;
-    ctx->info[6] = (use_simple_only ? 0 : 1) | ((int)global_hist << 2) | (box_type << 4) | (tri << 8) | ((int)split << 12) | ((int)big << 13) | ((int64_t)tj << 16);
+    const int form = box_type == CDH_BOX_ORTHO ? ((ctx->flags & CDH_FLAG_NO_PRUNE) ? ORTHO_PLAIN : fused_ok ? ORTHO_FUSED : ORTHO_EXACT) : tri;
+    ctx->info[6] = (use_simple_only ? 0 : 1) | ((int)global_hist << 2) | (box_type << 4) | (form << 8) | ((int)split << 12) | ((int)big << 13) | ((int64_t)tj << 16);
     ctx->info[7] = (int64_t)wt.padded_pairs;
     return CDH_OK;
 }

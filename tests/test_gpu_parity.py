@@ -141,10 +141,24 @@ def test_ortho_awkward_box_lengths_fused_and_plain_rint(seed):
     g = np.random.Generator(np.random.PCG64(seed))
     L = g.uniform(3.0, 40.0, size=3) * np.array([1.0, 1.0 / 3.0, math.pi])
     p = inputs.uniform_problem(seed, (1500, 2100), inputs.BOX_ORTHO, 5000, 0.5 * float(L.min()), box=np.diag(L))
-    a, _ = gpu_hist(p)
-    b, _ = gpu_hist(p, cdh.FLAG_NO_PRUNE)
-    assert_same(a, oracle_hist(p), f"fused rint, L={L}")
-    assert_same(b, a, "plain vs fused rint")
+    a, info_a = gpu_hist(p)
+    b, info_b = gpu_hist(p, cdh.FLAG_NO_PRUNE)
+    assert info_a["form"] in (1, 2) and info_b["form"] == 0      # fused or exact-product form vs the pinned 5-operation form
+    assert_same(a, oracle_hist(p), f"rint form {info_a['form']}, L={L}")
+    assert_same(b, a, "plain vs fused / exact-product rint")
+
+
+def test_ortho_rint_forms_all_occur():
+    # over a handful of seeded boxes both the fused form (constants found for all axes) and the exact-product form occur
+    forms = set()
+    for seed in range(50, 62):
+        g = np.random.Generator(np.random.PCG64(seed))
+        L = g.uniform(3.0, 40.0, size=3)
+        p = inputs.uniform_problem(seed, (700, 900), inputs.BOX_ORTHO, 3000, 0.5 * float(L.min()), box=np.diag(L))
+        got, info = gpu_hist(p)
+        forms.add(info["form"])
+        assert_same(got, oracle_hist(p), f"form {info['form']} L={L}")
+    assert forms == {1, 2}
 
 
 def test_ortho_pairs_on_the_half_box_switch_point():
