@@ -60,6 +60,9 @@ extern "C" {
                                               (measurement; read with cdh_last_call_kernel_ms) */
 #define CDH_FLAG_GLOBAL_HIST      (1u << 5) /* no private histogram: every kept pair adds to the uint64 result
                                               directly (chosen automatically for very wide histograms) */
+#define CDH_FLAG_ACCUMULATE       (1u << 6) /* cdh_histograms ADDS to `out` instead of overwriting it: a caller can feed a
+                                              trajectory in chunks of frames (the paper's writer sums every 100 frames,
+                                              PAPER.md:338).  Not for cdh_histograms_host (its device result is scratch) */
 #define CDH_FLAG_MAX_SMEM_BINS_SHIFT 8     /* bits 8..31: if non-zero, cap on the bins one CTA keeps in
                                               shared memory (forces the bin-range-split path) */
 
@@ -93,7 +96,8 @@ int cdh_create(cdh_ctx **ctx, int device, uint32_t flags);
  *  precision       CDH_F32 or CDH_F64 (constants are then used in double: r_max, n_bins / r_max, the box).
  *  stream          cudaStream_t (as void*), may be 0.  All work is enqueued on it; the call does not
  *                  synchronise.  `out` is valid once the caller has synchronised the stream.
- *  out             DEVICE pointer, uint64 [n_species*(n_species+1)/2][n_bins], OVERWRITTEN.
+ *  out             DEVICE pointer, uint64 [n_species*(n_species+1)/2][n_bins], OVERWRITTEN (added to with
+ *                  CDH_FLAG_ACCUMULATE).
  *                  Row index of species pair (p <= q): p*n_species - p*(p-1)/2 + (q - p).
  *
  * Host arrays are read during the call only.  Returns CDH_OK or a negative code; on

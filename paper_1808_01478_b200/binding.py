@@ -25,6 +25,7 @@ FLAG_WARP_AGGREGATE = 1 << 2
 FLAG_NO_AGGREGATE = 1 << 3
 FLAG_TIME_KERNELS = 1 << 4
 FLAG_GLOBAL_HIST = 1 << 5
+FLAG_ACCUMULATE = 1 << 6
 FLAG_MAX_SMEM_BINS_SHIFT = 8
 
 EXPORTS = ["cdh_create", "cdh_histograms", "cdh_histograms_host", "cdh_destroy", "cdh_strerror",

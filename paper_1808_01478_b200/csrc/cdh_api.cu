@@ -290,7 +290,8 @@ static int histograms_f64(cdh_ctx* ctx, const double* coords, int32_t n_frames, 
     CDH_CUDA(cudaEventRecord(ctx->staged, stream));
     ctx->staged_pending = true;
     CDH_CUDA(cudaMemsetAsync(ctx->d_scalars, 0, 64, stream));
-    CDH_CUDA(cudaMemsetAsync(out, 0, (size_t)n_hist * (size_t)n_bins * sizeof(uint64_t), stream));
+    if (!(ctx->flags & CDH_FLAG_ACCUMULATE))
+        CDH_CUDA(cudaMemsetAsync(out, 0, (size_t)n_hist * (size_t)n_bins * sizeof(uint64_t), stream));
 
     int launches = 0;
     if (frame_slots > 0) {
@@ -477,7 +478,8 @@ extern "C" int cdh_histograms(cdh_ctx* ctx, const void* coords, int32_t n_frames
     CDH_CUDA(cudaEventRecord(ctx->staged, stream));
     ctx->staged_pending = true;
     CDH_CUDA(cudaMemsetAsync(ctx->d_scalars, 0, 64, stream));
-    CDH_CUDA(cudaMemsetAsync(out, 0, (size_t)n_hist * (size_t)n_bins * sizeof(uint64_t), stream));
+    if (!(ctx->flags & CDH_FLAG_ACCUMULATE))
+        CDH_CUDA(cudaMemsetAsync(out, 0, (size_t)n_hist * (size_t)n_bins * sizeof(uint64_t), stream));
 
     int launches = 0;
     // ---- K0 repack -----------------------------------------------------------------------------
@@ -546,8 +548,11 @@ extern "C" int cdh_histograms_host(cdh_ctx* ctx, const void* coords, int32_t n_f
     if ((rc = grow(ctx, &ctx->d_io_coords, &ctx->io_coords_bytes, cbytes > 0 ? cbytes : 16, false)) != CDH_OK) return rc;
     if ((rc = grow(ctx, &ctx->d_io_out, &ctx->io_out_bytes, obytes, false)) != CDH_OK) return rc;
     if (cbytes) CDH_CUDA(cudaMemcpyAsync(ctx->d_io_coords, coords, cbytes, cudaMemcpyHostToDevice, stream));   // one H2D copy
+    const uint32_t saved_flags = ctx->flags;
+    ctx->flags &= ~CDH_FLAG_ACCUMULATE;                       // the device result of this entry point is scratch: overwrite
     rc = cdh_histograms(ctx, ctx->d_io_coords, n_frames, off, n_species, box_type, box, n_boxes, r_max, n_bins,
                         precision, stream_, (uint64_t*)ctx->d_io_out);
+    ctx->flags = saved_flags;
     if (rc != CDH_OK) return rc;
     CDH_CUDA(cudaMemcpyAsync(out, ctx->d_io_out, obytes, cudaMemcpyDeviceToHost, stream));                      // one D2H copy
     CDH_CUDA(cudaStreamSynchronize(stream));

@@ -360,3 +360,16 @@ def test_periodic_boxes_far_from_the_origin():
                                p.box_type, p.box, p.r_max, p.n_bins)
             got, info = gpu_hist(q)
             assert_same(got, oracle_hist(q), f"box_type {p.box_type} shifted by {shift} {info}")
+
+
+def test_accumulate_flag_sums_chunks_of_a_trajectory():
+    _need_gpu()
+    p = inputs.reduced_config(4)                     # 3 frames
+    dev = torch.device("cuda", 0)
+    out = torch.zeros((p.n_hist, p.n_bins), dtype=torch.int64, device=dev)
+    with cdh.Context(0, cdh.FLAG_ACCUMULATE) as ctx:
+        for f in range(p.n_frames):                  # one frame per call, all into the same result
+            c = torch.from_numpy(np.ascontiguousarray(p.coords[f:f + 1])).to(dev)
+            ctx.cdh_histograms(c, 1, p.species_offsets, p.box_type, p.box, p.r_max, p.n_bins, out)
+        torch.cuda.synchronize()
+    assert_same(out.cpu().numpy().view(np.uint64), oracle_hist(p), "accumulated over three calls")
