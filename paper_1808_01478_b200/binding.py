@@ -30,7 +30,8 @@ FLAG_MAX_SMEM_BINS_SHIFT = 8
 
 EXPORTS = ["cdh_create", "cdh_histograms", "cdh_histograms_host", "cdh_destroy", "cdh_strerror",
            "cdh_last_error", "cdh_last_call_info", "cdh_call_kernel_ms", "cdh_rdf",
-           "cdh_bench_fp32_rate", "cdh_bench_shared_atomics", "cdh_selftest_sqrt", "cdh_selftest_sqrt_f64"]
+           "cdh_bench_fp32_rate", "cdh_bench_shared_atomics", "cdh_selftest_sqrt", "cdh_selftest_sqrt_f64",
+           "cdh_host_d2_threshold_bits", "cdh_host_fused_rint_constant", "cdh_host_work_items"]
 
 
 class CdhError(RuntimeError):
@@ -80,6 +81,12 @@ def load(path: Optional[str] = None) -> ctypes.CDLL:
                                              ctypes.POINTER(dbl), ctypes.POINTER(dbl), ctypes.POINTER(dbl)]
     lib.cdh_selftest_sqrt.restype = ctypes.c_int
     lib.cdh_selftest_sqrt.argtypes = [u32, u32, vp, ctypes.POINTER(ctypes.c_uint64)]
+    lib.cdh_host_d2_threshold_bits.restype = ctypes.c_uint32
+    lib.cdh_host_d2_threshold_bits.argtypes = [ctypes.c_float]
+    lib.cdh_host_fused_rint_constant.restype = ctypes.c_int
+    lib.cdh_host_fused_rint_constant.argtypes = [ctypes.c_float, ctypes.POINTER(ctypes.c_float)]
+    lib.cdh_host_work_items.restype = ctypes.c_int64
+    lib.cdh_host_work_items.argtypes = [i32, vp, i32, i32, i32, i32, i32, vp, ctypes.c_int64]
     lib.cdh_selftest_sqrt_f64.restype = ctypes.c_int
     lib.cdh_selftest_sqrt_f64.argtypes = [ctypes.c_uint64, ctypes.c_uint64, vp, ctypes.POINTER(ctypes.c_uint64)]
     if path is None:

@@ -588,3 +588,43 @@ extern "C" int cdh_rdf(cdh_ctx* ctx, const uint64_t* hist, int32_t n_hist, int32
     CDH_CUDA(cudaGetLastError());
     return CDH_OK;
 }
+
+// ---- host-logic hooks (include/cdh_bench.h): no device is touched, usable on a machine without a GPU ---------------
+extern "C" uint32_t cdh_host_d2_threshold_bits(float rmax) { return d2_threshold_bits(rmax); }
+
+extern "C" int cdh_host_fused_rint_constant(float inv_l, float* inv_lf) {
+    return (inv_lf && fused_rint_constant(inv_l, inv_lf)) ? 1 : 0;
+}
+
+extern "C" int64_t cdh_host_work_items(int32_t n_frames, const int32_t* off, int32_t n_species, int32_t n_bins,
+                                       int32_t cap_bins, int32_t ti, int32_t tj, int64_t* items, int64_t max_items) {
+    if (!off || n_frames < 1 || n_species < 1 || n_bins < 1 || cap_bins < 1 || ti < 4 || tj < kStageParticles ||
+        tj % kStageParticles || (max_items > 0 && !items))
+        return -1;
+    std::vector<uint32_t> pad_off((size_t)n_species + 1);
+    uint64_t slots = 0;
+    for (int s = 0; s < n_species; ++s) {
+        pad_off[s] = (uint32_t)slots;
+        slots += ((uint64_t)(off[s + 1] - off[s]) + kPadParticles - 1) / kPadParticles * kPadParticles;
+    }
+    pad_off[n_species] = (uint32_t)slots;
+    const SweepPlan sp = plan_sweeps((uint32_t)n_bins, (uint32_t)cap_bins);
+    WorkTables wt;
+    build_tables(n_frames, off, n_species, 1, (uint32_t)n_bins, sp, (uint32_t)ti, (uint32_t)tj, pad_off, (uint32_t)slots, &wt);
+    // expand the rows exactly as the tile kernel does: item -> (row, j-chunk)
+    int64_t n = 0;
+    for (size_t r = 0; r + 1 < wt.rows.size(); ++r) {
+        const Row& row = wt.rows[r];
+        const Seg& seg = wt.segs[row.seg];
+        const uint32_t count = wt.rows[r + 1].item_prefix - row.item_prefix;
+        for (uint32_t k = 0; k < count; ++k, ++n) {
+            if (n >= max_items) continue;
+            const uint32_t j0 = (row.jc0 + k) * (uint32_t)tj;
+            const uint32_t j1 = std::min((uint32_t)seg.nj, j0 + (uint32_t)tj);
+            int64_t* it = items + 8 * n;
+            it[0] = seg.hist; it[1] = seg.bin_lo; it[2] = seg.bin_cnt; it[3] = row.i0; it[4] = j0; it[5] = j1;
+            it[6] = seg.same; it[7] = ((int64_t)seg.i_group << 32) | seg.j_group;
+        }
+    }
+    return n == (int64_t)wt.n_items ? n : -2;
+}
