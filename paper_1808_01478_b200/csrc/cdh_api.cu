@@ -236,20 +236,22 @@ static int histograms_f64(cdh_ctx* ctx, const double* coords, int32_t n_frames, 
     uint32_t cap_bins = (uint32_t)((ctx->max_smem_optin - tile_smem_bytes64(0)) / 4);
     const uint32_t flag_cap = ctx->flags >> CDH_FLAG_MAX_SMEM_BINS_SHIFT;
     if (flag_cap && flag_cap < cap_bins) cap_bins = flag_cap;
-    const SweepPlan sp = plan_sweeps((uint32_t)n_bins, cap_bins);
-    const int smem_bytes = tile_smem_bytes64((int)sp.bins_per_sweep);
+    SweepPlan sp = plan_sweeps((uint32_t)n_bins, cap_bins);
+    const bool global_hist = (ctx->flags & CDH_FLAG_GLOBAL_HIST) != 0 || (!flag_cap && sp.n_sweeps >= kGlobalSweeps);
+    if (global_hist) { sp.n_sweeps = 1; sp.bins_per_sweep = (uint32_t)n_bins; }
+    const int smem_bytes = tile_smem_bytes64(global_hist ? 0 : (int)sp.bins_per_sweep);
     const bool big = 2 * (smem_bytes + 1024) > 228 * 1024;
     TileFn64 fn; int threads;
     const bool pbox = box_type == CDH_BOX_TRICLINIC && nb == 1;      // one box: constants through the parameter bank
-    const bool split64 = sp.n_sweeps > 1;
-    auto pick64 = [&](auto split_c) -> TileFn64 {
-        constexpr bool S = decltype(split_c)::value;
-        if (box_type == CDH_BOX_NONE) return big ? tile_kernel_f64<BOX_NONE, 512, 1, false, S> : tile_kernel_f64<BOX_NONE, 256, 2, false, S>;
-        if (box_type == CDH_BOX_ORTHO) return big ? tile_kernel_f64<BOX_ORTHO, 512, 1, false, S> : tile_kernel_f64<BOX_ORTHO, 256, 2, false, S>;
-        if (pbox) return big ? tile_kernel_f64<BOX_TRI, 512, 1, true, S> : tile_kernel_f64<BOX_TRI, 256, 2, true, S>;
-        return big ? tile_kernel_f64<BOX_TRI, 512, 1, false, S> : tile_kernel_f64<BOX_TRI, 256, 2, false, S>;
+    auto pick64 = [&](auto mode_c) -> TileFn64 {
+        constexpr int M = decltype(mode_c)::value;
+        if (box_type == CDH_BOX_NONE) return big ? tile_kernel_f64<BOX_NONE, 512, 1, false, M> : tile_kernel_f64<BOX_NONE, 256, 2, false, M>;
+        if (box_type == CDH_BOX_ORTHO) return big ? tile_kernel_f64<BOX_ORTHO, 512, 1, false, M> : tile_kernel_f64<BOX_ORTHO, 256, 2, false, M>;
+        if (pbox) return big ? tile_kernel_f64<BOX_TRI, 512, 1, true, M> : tile_kernel_f64<BOX_TRI, 256, 2, true, M>;
+        return big ? tile_kernel_f64<BOX_TRI, 512, 1, false, M> : tile_kernel_f64<BOX_TRI, 256, 2, false, M>;
     };
-    fn = split64 ? pick64(std::true_type{}) : pick64(std::false_type{});
+    fn = global_hist ? pick64(std::integral_constant<int, MODE_GLOBAL>{})
+       : sp.n_sweeps > 1 ? pick64(std::integral_constant<int, MODE_SPLIT>{}) : pick64(std::integral_constant<int, MODE_SHARED>{});
     threads = big ? 512 : 256;
     const uint32_t ti = (uint32_t)threads * kR;
     CDH_CUDA(cudaFuncSetAttribute((const void*)fn, cudaFuncAttributeMaxDynamicSharedMemorySize, smem_bytes));
@@ -318,7 +320,7 @@ static int histograms_f64(cdh_ctx* ctx, const double* coords, int32_t n_frames, 
         tp.boxes = (const BoxConst64*)(d + b_segs + b_rows);
         tp.counter = ctx->d_scalars; tp.out = (unsigned long long*)out; tp.range_keys = ctx->d_scalars + 4;
         tp.n_rows = (uint32_t)wt.rows.size() - 1; tp.n_items = (uint32_t)wt.n_items;
-        tp.n_bins = (uint32_t)n_bins; tp.tj = tj; tp.smem_bins = sp.bins_per_sweep;
+        tp.n_bins = (uint32_t)n_bins; tp.tj = tj; tp.smem_bins = global_hist ? 0u : sp.bins_per_sweep;
         tp.rmax = r_max; tp.scale = (double)n_bins / r_max;
         tp.box0 = boxes[0];
         grid = grid_full < tp.n_items ? grid_full : tp.n_items;
@@ -333,7 +335,7 @@ static int histograms_f64(cdh_ctx* ctx, const double* coords, int32_t n_frames, 
     }
     ctx->info[0] = launches; ctx->info[1] = (int64_t)wt.n_items; ctx->info[2] = sp.n_sweeps; ctx->info[3] = grid;
     ctx->info[4] = threads; ctx->info[5] = smem_bytes;
-    ctx->info[6] = 2 | (box_type << 4) | ((int)(sp.n_sweeps > 1) << 12) | ((int)big << 13) | ((int64_t)tj << 16);
+    ctx->info[6] = 2 | ((int)global_hist << 2) | (box_type << 4) | ((int)(sp.n_sweeps > 1) << 12) | ((int)big << 13) | ((int64_t)tj << 16);
     ctx->info[7] = (int64_t)wt.padded_pairs;
     return CDH_OK;
 }

@@ -151,19 +151,21 @@ __device__ __forceinline__ double pair_d2_f64(double xi, double yi, double zi, d
     return __dadd_rn(__dadd_rn(__dmul_rn(dx, dx), __dmul_rn(dy, dy)), __dmul_rn(dz, dz));
 }
 
-template <bool SPLIT>
+template <int MODE>
 __device__ __forceinline__ void bin_f64(double d2, double rmax, double scale, uint32_t last_bin, uint32_t hist,
-                                        uint32_t bin_lo, uint32_t lim, uint32_t trash, bool keep) {
+                                        uint32_t bin_lo, uint32_t lim, uint32_t trash, bool keep,
+                                        unsigned long long* __restrict__ grow) {
     const double d = sqrt_rn_f64(d2);
     const uint32_t f = __double2uint_rd(__dmul_rn(d, scale));   // floor, saturating (one F2I)
     const uint32_t b = min(f, last_bin) - bin_lo;               // reading Q3; unsigned wrap for bins below the sweep
     bool ok = keep && (d < rmax);                               // false for NaN (NaN input, +inf)
-    if constexpr (SPLIT) ok = ok && b < lim;
+    if constexpr (MODE == MODE_GLOBAL) { if (ok) atomicAdd(grow + b, 1ull); return; }    // bin_lo = 0 in this mode
+    if constexpr (MODE == MODE_SPLIT) ok = ok && b < lim;
     hist_inc(ok ? hist + 4u * b : trash);
 }
 
 // ---- K1 for doubles: same schedule, stages and flush rule as tile_kernel (cdh_tile.cuh) ------------
-template <int BOX, int T, int MINB, bool PBOX, bool SPLIT>
+template <int BOX, int T, int MINB, bool PBOX, int MODE>
 __global__ void __launch_bounds__(T, MINB) tile_kernel_f64(const TileParams64 P) {
     extern __shared__ __align__(128) unsigned char smem[];
     constexpr int TI = T * kR;
@@ -189,7 +191,7 @@ __global__ void __launch_bounds__(T, MINB) tile_kernel_f64(const TileParams64 P)
 
     auto flush = [&]() {
         __syncthreads();
-        if (cur_key != 0xFFFFFFFFu) {
+        if (MODE != MODE_GLOBAL && cur_key != 0xFFFFFFFFu) {
             unsigned long long* o = P.out + (size_t)cur_hist * P.n_bins;
             for (uint32_t b = tid; b < cur_lim; b += T) {
                 const uint32_t v = s_hist[b];
@@ -244,6 +246,7 @@ __global__ void __launch_bounds__(T, MINB) tile_kernel_f64(const TileParams64 P)
         const uint32_t s_begin = (masked && i0 > j0) ? (i0 - j0) / kStageParticles : 0;
         const double* jsrc = P.pk + ((size_t)seg.j_group + (j0 >> 2)) * kGroupFloats;
         const bool prune = (BOX == BOX_TRI) ? (range_ok && s_box->prune_ok != 0.0) : true;
+        unsigned long long* const grow = P.out + (size_t)seg.hist * P.n_bins;     // MODE_GLOBAL: the result row itself
         OrthoRegs64 ob;
         if constexpr (BOX == BOX_ORTHO) {
 #pragma unroll
@@ -284,7 +287,7 @@ __global__ void __launch_bounds__(T, MINB) tile_kernel_f64(const TileParams64 P)
                                 double d2;
                                 if constexpr (PBOX) d2 = pair_d2_f64<BOX>(xi[r], yi[r], zi[r], xj[c], yj[c], zj[c], P.box0, ob, prune);
                                 else d2 = pair_d2_f64<BOX>(xi[r], yi[r], zi[r], xj[c], yj[c], zj[c], *s_box, ob, prune);
-                                bin_f64<SPLIT>(d2, P.rmax, P.scale, P.n_bins - 1u, hist_addr, cur_lo, cur_lim, trash_addr, keep);
+                                bin_f64<MODE>(d2, P.rmax, P.scale, P.n_bins - 1u, hist_addr, cur_lo, cur_lim, trash_addr, keep, grow);
                             }
                     }
                 }

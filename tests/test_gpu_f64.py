@@ -149,3 +149,17 @@ def test_f64_ortho_half_box_switch_points():
         ctx.cdh_histograms(d, 1, off, inputs.BOX_ORTHO, box, 30.0, 1 << 20, out, precision=cdh.F64)
         torch.cuda.synchronize()
     same(out.cpu().numpy().view(np.uint64), want, "f64 pairs within 6 ulp of L/2")
+
+
+def test_f64_wide_histogram_global_and_split():
+    p = inputs.uniform_problem(19, (4000,), inputs.BOX_NONE, 800_000, math.sqrt(3.0))
+    want = oracle64(p)
+    a, info = gpu64(p)
+    assert info["global_hist"] and info["sweeps"] == 1
+    same(a, want, f"f64 800k bins, global histogram {info}")
+    b, info = gpu64(p, 45000 << cdh.FLAG_MAX_SMEM_BINS_SHIFT)
+    assert not info["global_hist"] and info["sweeps"] == 18
+    same(b, want, f"f64 800k bins, 18 sweeps {info}")
+    q = inputs.reduced_config(3)
+    c, info = gpu64(q, cdh.FLAG_GLOBAL_HIST)
+    same(c, oracle64(q), "f64 triclinic, forced global histogram")
