@@ -53,13 +53,15 @@ struct Row {
 // Per-box constants in fp32, derived on the host in double and rounded once (DESIGN.md
 // "Host-derived constants").  B has the box vectors as COLUMNS (Eq. 5).
 struct BoxConst {
+    float S[27][4];             // TRICLINIC: shift vectors ((i*B[r][0] + j*B[r][1]) + k*B[r][2]), i,j,k in -1..1; [3] = 0
+                                // (first member: 16-byte aligned in shared memory, one LDS.128 per shift)
     float L[3], invL[3];        // ORTHO
     float invLf[3];             // ORTHO_FUSED: the constant of the fused rint (host search, fused_rint_constant)
     float B[9], Binv[9];        // TRICLINIC, row-major
-    float S[27][3];             // TRICLINIC: shift vectors ((i*B[r][0] + j*B[r][1]) + k*B[r][2]), i,j,k in -1..1
-    float prune_ok;             // 1: r_max <= h_min/2 with margin, the zero-shift candidate may be tested alone
-    float pad_[3];
+    float prune_ok;             // TRICLINIC 1: r_max <= h_min/2 with margin, the zero-shift candidate may be tested alone
+                                // ORTHO 1: fused rint constants exist for all three axes
 };
+static_assert(sizeof(BoxConst) % 16 == 0, "BoxConst is copied and indexed in 16-byte units");
 
 struct TileParams {
     const float*    pk;         // repacked coordinates

@@ -185,16 +185,23 @@ __global__ void __launch_bounds__(T, MINB) tile_kernel(const TileParams P) {
                             }
                         }
                         if constexpr (BOX == BOX_TRI) {
-                            // rare: some element of the group has a fractional coordinate within kPruneDelta of
-                            // +-1/2 (or pruning is off for this box / r_max): run the definition for those elements
-                            if (!prune || fm_all > kPruneLimit) {
+                            if (!prune) {
+                                // pruning is off for this box / r_max: the definition for every pair, packed
+#pragma unroll
+                                for (int r = 0; r < kR; ++r) {
+                                    D2[r][0] = pair_d2_full_packed<TRI>(XA, YA, ZA, xi[r], yi[r], zi[r], fb, s_box, ONE);
+                                    D2[r][1] = pair_d2_full_packed<TRI>(XB, YB, ZB, xi[r], yi[r], zi[r], fb, s_box, ONE);
+                                }
+                            } else if (fm_all > kPruneLimit) {
+                                // rare: some element of the group has a fractional coordinate within kPruneDelta of
+                                // +-1/2: run the definition for those elements, out of line
                                 const float xj[4] = {XJ.x, XJ.y, XJ.z, XJ.w}, yj[4] = {YJ.x, YJ.y, YJ.z, YJ.w}, zj[4] = {ZJ.x, ZJ.y, ZJ.z, ZJ.w};
 #pragma unroll
                                 for (int r = 0; r < kR; ++r) {
 #pragma unroll
                                     for (int hlf = 0; hlf < 2; ++hlf) {
                                         float p, q; upk2(D2[r][hlf], p, q);
-                                        bool n0 = !prune || fm[r][hlf][0] > kPruneLimit, n1 = !prune || fm[r][hlf][1] > kPruneLimit;
+                                        bool n0 = fm[r][hlf][0] > kPruneLimit, n1 = fm[r][hlf][1] > kPruneLimit;
                                         if constexpr (MASKED) { n0 = n0 && (jg + 2 * hlf > ig + r); n1 = n1 && (jg + 2 * hlf + 1 > ig + r); }
                                         if (n0) p = tri_full_d2(xi[r], yi[r], zi[r], xj[2 * hlf], yj[2 * hlf], zj[2 * hlf], s_box);
                                         if (n1) q = tri_full_d2(xi[r], yi[r], zi[r], xj[2 * hlf + 1], yj[2 * hlf + 1], zj[2 * hlf + 1], s_box);
