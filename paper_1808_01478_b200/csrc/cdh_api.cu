@@ -95,6 +95,9 @@ Variant pick_fast(int box_type, int tri, bool big) {      // tri: TRI_* for TRIC
              : tri == ORTHO_EXACT ? fast_variant<BOX_ORTHO, ORTHO_EXACT, SPLIT>(big) : fast_variant<BOX_ORTHO, ORTHO_PLAIN, SPLIT>(big);
     if (tri == TRI_UPPER_B01) return fast_variant<BOX_TRI, TRI_UPPER_B01, SPLIT>(big);
     if (tri == TRI_UPPER) return fast_variant<BOX_TRI, TRI_UPPER, SPLIT>(big);
+    if (tri == (TRI_UPPER_B01 | TRI_WIDE)) return fast_variant<BOX_TRI, TRI_UPPER_B01 | TRI_WIDE, SPLIT>(big);
+    if (tri == (TRI_UPPER | TRI_WIDE)) return fast_variant<BOX_TRI, TRI_UPPER | TRI_WIDE, SPLIT>(big);
+    if (tri == (TRI_GENERAL | TRI_WIDE)) return fast_variant<BOX_TRI, TRI_GENERAL | TRI_WIDE, SPLIT>(big);
     return fast_variant<BOX_TRI, TRI_GENERAL, SPLIT>(big);
 }
 template <int VAR>
@@ -417,9 +420,10 @@ extern "C" int cdh_histograms(cdh_ctx* ctx, const void* coords, int32_t n_frames
     // Launch plan: every tile launch of the call owns an interval (lo, hi] of the fractional-coordinate range the
     // repack kernel measures, and exactly one of them does the work (cdh_tile.cuh).
     //   ORTHO: fused rint up to 1.49 (exact-product form if the host found no fused constants for some box),
-    //          magic-number rint up to 2^20, library rintf beyond;  TRICLINIC: fast path up to 1.49 (n in {-1,0,1}), definition beyond.
+    //          magic-number rint up to 2^20, library rintf beyond;  TRICLINIC: fast path up to 1.49 (n in {-1,0,1}), wide fast path up to 64,
+    //          definition beyond.
     struct Launch { Variant v; float lo, hi; };
-    const float kInf = INFINITY, kSmall = 1.49f, kMagic = 1048576.0f;
+    const float kInf = INFINITY, kSmall = 1.49f, kWide = 64.0f, kMagic = 1048576.0f;
     bool fused_ok = box_type == CDH_BOX_ORTHO;
     for (int b = 0; b < nb && fused_ok; ++b) fused_ok = boxes[b].prune_ok != 0.0f;
     if (ctx->flags & CDH_FLAG_NO_PRUNE) fused_ok = false;          // tests: force the plain magic-number form
@@ -438,7 +442,8 @@ extern "C" int cdh_histograms(cdh_ctx* ctx, const void* coords, int32_t n_frames
         plan.push_back({vs, kMagic, kInf});
     } else {
         plan.push_back({fast_of(tri), -kInf, kSmall});
-        plan.push_back({vs, kSmall, kInf});
+        plan.push_back({fast_of(tri | TRI_WIDE), kSmall, kWide});      // unwrapped coordinates, up to 64 cells
+        plan.push_back({vs, kWide, kInf});
     }
     const Variant vf = plan[0].v;
     const uint32_t ti = (uint32_t)vf.threads * kR;

@@ -32,6 +32,9 @@ constexpr int MODE_SHARED = 0, MODE_SPLIT = 1, MODE_GLOBAL = 2;
 // at most the sign of a zero, never d2): 0 general 3x3, 1 upper triangular (a along x, b in the xy
 // plane), 2 upper triangular with B[0][1] == 0 as well (the rhombic dodecahedron of config 3).
 constexpr int TRI_GENERAL = 0, TRI_UPPER = 1, TRI_UPPER_B01 = 2;
+// + TRI_WIDE: coordinates spanning up to 64 cells (unwrapped trajectories): n_k is no longer in {-1,0,1}, so B*n uses the
+// pinned multiply / add chain and the pruning margin grows with the measured range (cdh_tile.cuh).
+constexpr int TRI_WIDE = 4;
 // For BOX_ORTHO the same template slot selects the rint form (cdh_fast.cuh): 0 the pinned 5-operation form, 1 fused
 // (3 operations per axis; needs the host-searched constants), 2 exact-product form (4 operations; n in {-1,0,1}).
 constexpr int ORTHO_PLAIN = 0, ORTHO_FUSED = 1, ORTHO_EXACT = 2;

@@ -44,10 +44,13 @@ __global__ void __launch_bounds__(T, MINB) tile_kernel(const TileParams P) {
     // The fast variants are exact only while the range of the fractional coordinates is small (fused rint and
     // exact B*n: n in {-1,0,1}; magic-number rint: |t| < 2^22).  Every launch of the call reads the range the
     // repack kernel measured and exactly one of them does the work (no host synchronisation).  Uniform over the grid.
+    float prune_lim = kPruneLimit;          // triclinic: the zero-shift candidate decides while max_k |s_k - n_k| <= prune_lim
     if constexpr (BOX != BOX_NONE) {
         const float range = frac_range(P.range_keys);
         const bool mine = !(range <= P.range_lo) && (range <= P.range_hi || P.range_hi == __int_as_float(0x7f800000));
         if (!mine) return;
+        // TRI_WIDE: the error of s_k grows linearly with the range, and so must the margin (2x the 2^-17 of range 1.49)
+        if constexpr (BOX == BOX_TRI && (TRI & TRI_WIDE) != 0) prune_lim = 0.5f - kPruneDelta * 2.0f * fmaxf(1.0f, range * (1.0f / 1.49f));
     }
 
     if (tid == 0) { mbar_init(bar_addr, 1); mbar_init(bar_addr + 8, 1); fence_mbar_init(); }
@@ -192,7 +195,7 @@ __global__ void __launch_bounds__(T, MINB) tile_kernel(const TileParams P) {
                                     D2[r][0] = pair_d2_full_packed<TRI>(XA, YA, ZA, xi[r], yi[r], zi[r], fb, s_box, ONE);
                                     D2[r][1] = pair_d2_full_packed<TRI>(XB, YB, ZB, xi[r], yi[r], zi[r], fb, s_box, ONE);
                                 }
-                            } else if (fm_all > kPruneLimit) {
+                            } else if (fm_all > prune_lim) {
                                 // rare: some element of the group has a fractional coordinate within kPruneDelta of
                                 // +-1/2: run the definition for those elements, out of line
                                 const float xj[4] = {XJ.x, XJ.y, XJ.z, XJ.w}, yj[4] = {YJ.x, YJ.y, YJ.z, YJ.w}, zj[4] = {ZJ.x, ZJ.y, ZJ.z, ZJ.w};
@@ -201,7 +204,7 @@ __global__ void __launch_bounds__(T, MINB) tile_kernel(const TileParams P) {
 #pragma unroll
                                     for (int hlf = 0; hlf < 2; ++hlf) {
                                         float p, q; upk2(D2[r][hlf], p, q);
-                                        bool n0 = fm[r][hlf][0] > kPruneLimit, n1 = fm[r][hlf][1] > kPruneLimit;
+                                        bool n0 = fm[r][hlf][0] > prune_lim, n1 = fm[r][hlf][1] > prune_lim;
                                         if constexpr (MASKED) { n0 = n0 && (jg + 2 * hlf > ig + r); n1 = n1 && (jg + 2 * hlf + 1 > ig + r); }
                                         if (n0) p = tri_full_d2(xi[r], yi[r], zi[r], xj[2 * hlf], yj[2 * hlf], zj[2 * hlf], s_box);
                                         if (n1) q = tri_full_d2(xi[r], yi[r], zi[r], xj[2 * hlf + 1], yj[2 * hlf + 1], zj[2 * hlf + 1], s_box);

@@ -373,3 +373,20 @@ def test_accumulate_flag_sums_chunks_of_a_trajectory():
             ctx.cdh_histograms(c, 1, p.species_offsets, p.box_type, p.box, p.r_max, p.n_bins, out)
         torch.cuda.synchronize()
     assert_same(out.cpu().numpy().view(np.uint64), oracle_hist(p), "accumulated over three calls")
+
+
+@pytest.mark.parametrize("spread", [1.6, 3.0, 12.0, 40.0, 90.0])
+def test_triclinic_unwrapped_coordinates_wide_tier(spread):
+    # coordinates spanning several cells (unwrapped trajectories): range 1.49 .. 64 takes the wide fast path (pinned B*n
+    # chain, pruning margin grown with the range), beyond 64 the plain kernel; all must equal the oracle
+    box = np.array([[9.0, 0.0, 0.0], [1.5, 8.0, 0.0], [-2.0, 2.5, 7.0]])
+    p = inputs.uniform_problem(88, (1500, 2300), inputs.BOX_TRICLINIC, 4000, 3.4, box=box, spread=spread)
+    got, info = gpu_hist(p)
+    assert_same(got, oracle_hist(p), f"triclinic spread {spread} {info}")
+    q = inputs.config3(counts=(1700, 2100), n_bins=5000)
+    g = np.random.Generator(np.random.PCG64(int(spread * 10)))
+    shifts = g.integers(-int(spread), int(spread) + 1, size=(q.n_total, 3)).astype(np.float64) @ q.box.reshape(3, 3)
+    q = inputs.Problem("cfg3_unwrapped", (q.coords.astype(np.float64) + shifts[None]).astype(np.float32), q.species_offsets,
+                       q.box_type, q.box, q.r_max, q.n_bins)
+    got, info = gpu_hist(q)
+    assert_same(got, oracle_hist(q), f"config 3 shifted by up to {int(spread)} cells {info}")
