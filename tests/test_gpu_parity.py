@@ -390,3 +390,25 @@ def test_triclinic_unwrapped_coordinates_wide_tier(spread):
                        q.box_type, q.box, q.r_max, q.n_bins)
     got, info = gpu_hist(q)
     assert_same(got, oracle_hist(q), f"config 3 shifted by up to {int(spread)} cells {info}")
+
+
+@pytest.mark.parametrize("r_max", [7.0, 12.0])
+def test_triclinic_pairs_on_the_half_cell_switch_points(r_max):
+    # fractional separations within a few ulps of 1/2 on each axis of a dyadic cell (all coordinates exact): exactly where
+    # Eq. 5 can pick the far image and where the pruning test has to hand the pair to the 27-shift search
+    box = np.array([[16.0, 0.0, 0.0], [0.0, 16.0, 0.0], [8.0, 8.0, 16.0]])        # heights 14.3, 14.3, 16
+    rows = [np.zeros(3)]
+    for ax in range(3):
+        for k in range(-8, 9):
+            for other in (0.0, 0.125, 0.4375):
+                s = np.array([other, other / 2, other / 4])
+                s[ax] = 0.5 + k * 2.0 ** -23
+                rows.append(s @ box)
+                rows.append(-(s @ box))
+    pts = np.array(rows, dtype=np.float32)[None]
+    p = inputs.Problem("tri_half", pts, np.array([0, 1, len(rows)], dtype=np.int32), inputs.BOX_TRICLINIC, box.reshape(1, 9),
+                       r_max, 1 << 16)
+    want = oracle_hist(p)
+    for flags in (0, cdh.FLAG_NO_PRUNE, cdh.FLAG_SIMPLE_KERNEL):
+        got, info = gpu_hist(p, flags)
+        assert_same(got, want, f"flags {flags:#x} {info}")
