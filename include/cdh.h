@@ -117,6 +117,26 @@ int cdh_histograms_host(cdh_ctx *ctx, const void *coords, int32_t n_frames,
                         const double *box, int32_t n_boxes, double r_max, int32_t n_bins,
                         int32_t precision, void *stream, uint64_t *out);
 
+/*
+ * cdh_histograms_host for a trajectory: the frames are processed in chunks of `frames_per_chunk` frames, the
+ * H2D copy of chunk c+1 (on a private copy stream, into the other of two chunk buffers) overlapping the kernels of
+ * chunk c on `stream`; every frame crosses the bus once and the chunks are summed on the device
+ * (Eq. 2; the paper's engine streams frames to the kernels the same way).  Device memory
+ * is two chunks instead of the whole trajectory, so the trajectory may be larger than the device memory.
+ *
+ *  coords            HOST pointer, [n_frames][n_total][3]; page-locked memory is needed for the copies to overlap
+ *                    (pageable memory works, the copies then pass through the driver's staging buffer).
+ *  frames_per_chunk  >= 1, or 0 = automatic (the fewest frames with 8e9 pairs, at most 1 GiB of coordinates).
+ *  box, n_boxes      as cdh_histograms; with n_boxes == n_frames chunk c uses its own frames' boxes.
+ *  out               HOST pointer, uint64 [n_hist][n_bins], overwritten.
+ * The result is independent of frames_per_chunk (integer sums).  cdh_last_call_info describes the last chunk.
+ * Synchronises `stream` before returning.  Other arguments, return codes and error behaviour as cdh_histograms_host.
+ */
+int cdh_histograms_stream(cdh_ctx *ctx, const void *coords, int32_t n_frames,
+                          const int32_t *species_offsets, int32_t n_species, int32_t box_type,
+                          const double *box, int32_t n_boxes, double r_max, int32_t n_bins,
+                          int32_t precision, int32_t frames_per_chunk, void *stream, uint64_t *out);
+
 /* Destroy the context and free its scratch (synchronises the device).  NULL is accepted. */
 int cdh_destroy(cdh_ctx *ctx);
 
@@ -131,7 +151,9 @@ const char *cdh_last_error(const cdh_ctx *ctx);
  *   info[2] = bin-range sweeps                   info[3] = CTAs of the tile kernel
  *   info[4] = threads per CTA                    info[5] = dynamic shared memory bytes per CTA
  *   info[6] = kernel variant id (bit 0 fast path, bit 2 global histogram, bits 4-7 box type, bits 8-11 form: ORTHO 0 plain /
- *             1 fused / 2 exact-product rint, TRICLINIC zero structure; bits 16.. j-chunk size)                  info[7] = evaluated pairs incl. padding lanes (low 32 bits unused; see info64)
+ *             1 fused / 2 exact-product rint, TRICLINIC zero structure; bit 12 bin-range split, bit 13 one-CTA-per-SM shape,
+ *             bit 14 small-species variant: warps skip below-diagonal and padding-only work; bits 16.. j-chunk size)
+ *   info[7] = pair slots the tile kernel is scheduled to walk (evaluated pairs incl. masked and padding lanes)
  * Returns CDH_OK or CDH_ERR_INVALID_ARG. */
 int cdh_last_call_info(const cdh_ctx *ctx, int64_t info[8]);
 

@@ -28,7 +28,7 @@ FLAG_GLOBAL_HIST = 1 << 5
 FLAG_ACCUMULATE = 1 << 6
 FLAG_MAX_SMEM_BINS_SHIFT = 8
 
-EXPORTS = ["cdh_create", "cdh_histograms", "cdh_histograms_host", "cdh_destroy", "cdh_strerror",
+EXPORTS = ["cdh_create", "cdh_histograms", "cdh_histograms_host", "cdh_histograms_stream", "cdh_destroy", "cdh_strerror",
            "cdh_last_error", "cdh_last_call_info", "cdh_call_kernel_ms", "cdh_rdf",
            "cdh_bench_fp32_rate", "cdh_bench_shared_atomics", "cdh_selftest_sqrt", "cdh_selftest_sqrt_f64",
            "cdh_host_d2_threshold_bits", "cdh_host_fused_rint_constant", "cdh_host_work_items"]
@@ -61,6 +61,8 @@ def load(path: Optional[str] = None) -> ctypes.CDLL:
     lib.cdh_histograms.argtypes = hist_args
     lib.cdh_histograms_host.restype = ctypes.c_int
     lib.cdh_histograms_host.argtypes = hist_args
+    lib.cdh_histograms_stream.restype = ctypes.c_int
+    lib.cdh_histograms_stream.argtypes = hist_args[:11] + [i32, vp, vp]
     lib.cdh_destroy.restype = ctypes.c_int
     lib.cdh_destroy.argtypes = [vp]
     lib.cdh_strerror.restype = ctypes.c_char_p
@@ -178,6 +180,33 @@ class Context:
         self._check(rc)
         return out
 
+    def cdh_histograms_stream(self, coords: np.ndarray, species_offsets: Sequence[int], box_type: int, box,
+                              r_max: float, n_bins: int, precision: int = F32, frames_per_chunk: int = 0,
+                              stream=None, out: Optional[np.ndarray] = None) -> np.ndarray:
+        """include/cdh.h ``cdh_histograms_stream``: HOST coords [n_frames, n_total, 3] (numpy, or a pinned CPU torch
+        tensor for overlapped copies) -> HOST uint64 [n_hist, n_bins]; frames go to the device chunk by chunk."""
+        want = np.float64 if precision == F64 else np.float32
+        if hasattr(coords, "data_ptr"):                      # torch tensor (pinned host memory)
+            if coords.is_cuda or not coords.is_contiguous():
+                raise ValueError("coords must be a contiguous CPU tensor")
+            shape, dt, addr = tuple(coords.shape), np.dtype(str(coords.dtype).replace("torch.", "")), coords.data_ptr()
+        else:
+            coords = np.ascontiguousarray(coords)
+            shape, dt, addr = coords.shape, coords.dtype, coords.ctypes.data
+        if dt != want or len(shape) != 3 or shape[2] != 3:
+            raise ValueError(f"coords must be {np.dtype(want).name} [n_frames, n_total, 3] for this precision")
+        off, b, n_boxes = self._marshal(species_offsets, box, shape[0])
+        n_species = len(off) - 1
+        n_hist = n_species * (n_species + 1) // 2
+        if out is None:
+            out = np.empty((n_hist, int(n_bins)), dtype=np.uint64)
+        rc = self._lib.cdh_histograms_stream(self._h, addr, int(shape[0]), off.ctypes.data, n_species,
+                                             int(box_type), None if b is None else b.ctypes.data, n_boxes,
+                                             float(r_max), int(n_bins), int(precision), int(frames_per_chunk),
+                                             _stream_ptr(stream), out.ctypes.data)
+        self._check(rc)
+        return out
+
     def cdh_rdf(self, hist, n_hist: int, n_bins: int, r_max: float, n_frames: int, n_pairs, volume: float, g,
                 stream=None) -> None:
         """include/cdh.h ``cdh_rdf``: hist (uint64) and g (float64) are DEVICE buffers [n_hist, n_bins]."""
@@ -193,7 +222,7 @@ class Context:
         self._check(self._lib.cdh_last_call_info(self._h, arr))
         v = list(arr)
         return {"launches": v[0], "items": v[1], "sweeps": v[2], "ctas": v[3], "threads": v[4],
-                "smem_bytes": v[5], "variant": v[6], "tj": v[6] >> 16, "fast": bool(v[6] & 1), "global_hist": bool(v[6] & 4), "form": (v[6] >> 8) & 15,
+                "smem_bytes": v[5], "variant": v[6], "tj": v[6] >> 16, "fast": bool(v[6] & 1), "global_hist": bool(v[6] & 4), "form": (v[6] >> 8) & 15, "skip": bool(v[6] & (1 << 14)),
                 "padded_pairs": v[7]}
 
     def call_kernel_ms(self, calls_back: int = 0):

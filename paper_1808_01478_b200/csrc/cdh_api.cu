@@ -24,6 +24,10 @@ struct cdh_ctx {
     bool staged_pending = false;
     void* d_io_coords = nullptr; size_t io_coords_bytes = 0;  // cdh_histograms_host staging
     void* d_io_out = nullptr;    size_t io_out_bytes = 0;
+    // cdh_histograms_stream: two chunk buffers filled on a private copy stream while the other is being processed
+    void* d_chunk[2] = {nullptr, nullptr}; size_t chunk_bytes[2] = {0, 0};
+    cudaStream_t copy_stream = nullptr;
+    cudaEvent_t copied[2] = {nullptr, nullptr}, consumed[2] = {nullptr, nullptr};
     cudaEvent_t* ev = nullptr;   // CDH_FLAG_TIME_KERNELS: ring of [CDH_TIMED_CALLS][4]: call begin, tile begin, tile end, call end
     uint64_t timed_calls = 0;
     std::string err;
@@ -61,6 +65,34 @@ int grow(cdh_ctx* ctx, void** p, size_t* have, size_t need, bool pinned_host) {
     return CDH_OK;
 }
 
+// Pairs one frame evaluates (all species pairs).
+static double frame_pairs(const int32_t* off, int32_t n_species) {
+    double tot = 0.0;
+    for (int p = 0; p < n_species; ++p) {
+        const double np_ = (double)(off[p + 1] - off[p]);
+        tot += 0.5 * np_ * (np_ - 1.0);
+        for (int q = p + 1; q < n_species; ++q) tot += np_ * (double)(off[q + 1] - off[q]);
+    }
+    return tot;
+}
+
+#ifndef CDH_SKIP_EFFICIENCY
+#define CDH_SKIP_EFFICIENCY 0.9   // the SKIP variants (cdh_tile.cuh) are taken when fewer than this share of the pair slots the
+                                  // 1024-particle i-tiles walk are pairs of the problem
+#endif
+// Small species: the share of the walked pair slots (1024-particle i-tiles: full diagonal blocks, padded last tiles) that are
+// pairs of the problem decides whether the SKIP variants of the 256-thread kernels pay.
+static bool small_species(const int32_t* off, int32_t n_species) {
+    const double ti256 = 256.0 * kR;
+    double walked = 0.0;
+    for (int p = 0; p < n_species; ++p) {
+        const double tiles = std::ceil((double)(off[p + 1] - off[p]) / ti256);
+        walked += 0.5 * tiles * (tiles + 1.0) * ti256 * ti256;
+        for (int q = p + 1; q < n_species; ++q) walked += tiles * ti256 * (double)(off[q + 1] - off[q]);
+    }
+    return walked > 0.0 && frame_pairs(off, n_species) < CDH_SKIP_EFFICIENCY * walked;
+}
+
 // ---- kernel table -----------------------------------------------------------------------------
 typedef void (*TileFn)(const TileParams);
 struct Variant { TileFn fn; int threads; };
@@ -82,23 +114,25 @@ constexpr uint64_t kItemsPerCta = CDH_ITEMS_PER_CTA;
 #define CDH_BIG_T 1024  // threads of the one-CTA-per-SM variants (32 warps/SM: config 5 +5 % over 512)
 #endif
 template <int BOX, int TRI, int MODE>
-Variant fast_variant(bool big) {
+Variant fast_variant(bool big, bool skip) {
     if constexpr (MODE != MODE_GLOBAL)
         if (big) return {tile_kernel<BOX, TRI, CDH_BIG_T, VAR_FAST, MODE, 1>, CDH_BIG_T};
+    if constexpr (MODE == MODE_SHARED)
+        if (skip) return {tile_kernel<BOX, TRI, 256, VAR_FAST, MODE, (BOX == BOX_TRI ? 2 : CDH_MINB), true>, 256};
     return {tile_kernel<BOX, TRI, 256, VAR_FAST, MODE, (BOX == BOX_TRI ? 2 : CDH_MINB)>, 256};
 }
 template <int SPLIT>
-Variant pick_fast(int box_type, int tri, bool big) {      // tri: TRI_* for TRICLINIC, ORTHO_* for ORTHO
-    if (box_type == CDH_BOX_NONE) return fast_variant<BOX_NONE, 0, SPLIT>(big);
+Variant pick_fast(int box_type, int tri, bool big, bool skip) {      // tri: TRI_* for TRICLINIC, ORTHO_* for ORTHO
+    if (box_type == CDH_BOX_NONE) return fast_variant<BOX_NONE, 0, SPLIT>(big, skip);
     if (box_type == CDH_BOX_ORTHO)
-        return tri == ORTHO_FUSED ? fast_variant<BOX_ORTHO, ORTHO_FUSED, SPLIT>(big)
-             : tri == ORTHO_EXACT ? fast_variant<BOX_ORTHO, ORTHO_EXACT, SPLIT>(big) : fast_variant<BOX_ORTHO, ORTHO_PLAIN, SPLIT>(big);
-    if (tri == TRI_UPPER_B01) return fast_variant<BOX_TRI, TRI_UPPER_B01, SPLIT>(big);
-    if (tri == TRI_UPPER) return fast_variant<BOX_TRI, TRI_UPPER, SPLIT>(big);
-    if (tri == (TRI_UPPER_B01 | TRI_WIDE)) return fast_variant<BOX_TRI, TRI_UPPER_B01 | TRI_WIDE, SPLIT>(big);
-    if (tri == (TRI_UPPER | TRI_WIDE)) return fast_variant<BOX_TRI, TRI_UPPER | TRI_WIDE, SPLIT>(big);
-    if (tri == (TRI_GENERAL | TRI_WIDE)) return fast_variant<BOX_TRI, TRI_GENERAL | TRI_WIDE, SPLIT>(big);
-    return fast_variant<BOX_TRI, TRI_GENERAL, SPLIT>(big);
+        return tri == ORTHO_FUSED ? fast_variant<BOX_ORTHO, ORTHO_FUSED, SPLIT>(big, skip)
+             : tri == ORTHO_EXACT ? fast_variant<BOX_ORTHO, ORTHO_EXACT, SPLIT>(big, skip) : fast_variant<BOX_ORTHO, ORTHO_PLAIN, SPLIT>(big, skip);
+    if (tri == TRI_UPPER_B01) return fast_variant<BOX_TRI, TRI_UPPER_B01, SPLIT>(big, skip);
+    if (tri == TRI_UPPER) return fast_variant<BOX_TRI, TRI_UPPER, SPLIT>(big, skip);
+    if (tri == (TRI_UPPER_B01 | TRI_WIDE)) return fast_variant<BOX_TRI, TRI_UPPER_B01 | TRI_WIDE, SPLIT>(big, skip);
+    if (tri == (TRI_UPPER | TRI_WIDE)) return fast_variant<BOX_TRI, TRI_UPPER | TRI_WIDE, SPLIT>(big, skip);
+    if (tri == (TRI_GENERAL | TRI_WIDE)) return fast_variant<BOX_TRI, TRI_GENERAL | TRI_WIDE, SPLIT>(big, skip);
+    return fast_variant<BOX_TRI, TRI_GENERAL, SPLIT>(big, skip);
 }
 template <int VAR>
 Variant simple_variant(int box_type, bool big) {
@@ -196,6 +230,12 @@ extern "C" int cdh_destroy(cdh_ctx* ctx) {
     if (ctx->h_tables) cudaFreeHost(ctx->h_tables);
     if (ctx->d_io_coords) cudaFree(ctx->d_io_coords);
     if (ctx->d_io_out) cudaFree(ctx->d_io_out);
+    for (int k = 0; k < 2; ++k) {
+        if (ctx->d_chunk[k]) cudaFree(ctx->d_chunk[k]);
+        if (ctx->copied[k]) cudaEventDestroy(ctx->copied[k]);
+        if (ctx->consumed[k]) cudaEventDestroy(ctx->consumed[k]);
+    }
+    if (ctx->copy_stream) cudaStreamDestroy(ctx->copy_stream);
     if (ctx->staged) cudaEventDestroy(ctx->staged);
     if (ctx->ev) {
         for (int k = 0; k < 4 * CDH_TIMED_CALLS; ++k) if (ctx->ev[k]) cudaEventDestroy(ctx->ev[k]);
@@ -246,8 +286,15 @@ static int histograms_f64(cdh_ctx* ctx, const double* coords, int32_t n_frames, 
     const bool big = 2 * (smem_bytes + 1024) > 228 * 1024;
     TileFn64 fn; int threads;
     const bool pbox = box_type == CDH_BOX_TRICLINIC && nb == 1;      // one box: constants through the parameter bank
+    const bool skip = !big && !global_hist && sp.n_sweeps == 1 && small_species(off, n_species);
     auto pick64 = [&](auto mode_c) -> TileFn64 {
         constexpr int M = decltype(mode_c)::value;
+        if constexpr (M == MODE_SHARED)
+            if (skip) {
+                if (box_type == CDH_BOX_NONE) return tile_kernel_f64<BOX_NONE, 256, 2, false, M, true>;
+                if (box_type == CDH_BOX_ORTHO) return tile_kernel_f64<BOX_ORTHO, 256, 2, false, M, true>;
+                return pbox ? tile_kernel_f64<BOX_TRI, 256, 2, true, M, true> : tile_kernel_f64<BOX_TRI, 256, 2, false, M, true>;
+            }
         if (box_type == CDH_BOX_NONE) return big ? tile_kernel_f64<BOX_NONE, 512, 1, false, M> : tile_kernel_f64<BOX_NONE, 256, 2, false, M>;
         if (box_type == CDH_BOX_ORTHO) return big ? tile_kernel_f64<BOX_ORTHO, 512, 1, false, M> : tile_kernel_f64<BOX_ORTHO, 256, 2, false, M>;
         if (pbox) return big ? tile_kernel_f64<BOX_TRI, 512, 1, true, M> : tile_kernel_f64<BOX_TRI, 256, 2, true, M>;
@@ -338,7 +385,8 @@ static int histograms_f64(cdh_ctx* ctx, const double* coords, int32_t n_frames, 
     }
     ctx->info[0] = launches; ctx->info[1] = (int64_t)wt.n_items; ctx->info[2] = sp.n_sweeps; ctx->info[3] = grid;
     ctx->info[4] = threads; ctx->info[5] = smem_bytes;
-    ctx->info[6] = 2 | ((int)global_hist << 2) | (box_type << 4) | ((int)(sp.n_sweeps > 1) << 12) | ((int)big << 13) | ((int64_t)tj << 16);
+    ctx->info[6] = 2 | ((int)global_hist << 2) | (box_type << 4) | ((int)(sp.n_sweeps > 1) << 12) | ((int)big << 13) | ((int)skip << 14) |
+                   ((int64_t)tj << 16);
     ctx->info[7] = (int64_t)wt.padded_pairs;
     return CDH_OK;
 }
@@ -427,9 +475,10 @@ extern "C" int cdh_histograms(cdh_ctx* ctx, const void* coords, int32_t n_frames
     bool fused_ok = box_type == CDH_BOX_ORTHO;
     for (int b = 0; b < nb && fused_ok; ++b) fused_ok = boxes[b].prune_ok != 0.0f;
     if (ctx->flags & CDH_FLAG_NO_PRUNE) fused_ok = false;          // tests: force the plain magic-number form
+    const bool skip = small_species(off, n_species);
     auto fast_of = [&](int form) {
-        return global_hist ? pick_fast<MODE_GLOBAL>(box_type, form, big)
-                           : split ? pick_fast<MODE_SPLIT>(box_type, form, big) : pick_fast<MODE_SHARED>(box_type, form, big);
+        return global_hist ? pick_fast<MODE_GLOBAL>(box_type, form, big, false)
+                           : split ? pick_fast<MODE_SPLIT>(box_type, form, big, false) : pick_fast<MODE_SHARED>(box_type, form, big, skip);
     };
     const Variant vs = global_hist ? simple_global(box_type) : pick_simple(box_type, big, ctx->flags);
     std::vector<Launch> plan;
@@ -536,7 +585,9 @@ extern "C" int cdh_histograms(cdh_ctx* ctx, const void* coords, int32_t n_frames
     ctx->info[0] = launches; ctx->info[1] = (int64_t)wt.n_items; ctx->info[2] = sp.n_sweeps; ctx->info[3] = grid;
     ctx->info[4] = vf.threads; ctx->info[5] = smem_bytes;
     const int form = box_type == CDH_BOX_ORTHO ? ((ctx->flags & CDH_FLAG_NO_PRUNE) ? ORTHO_PLAIN : fused_ok ? ORTHO_FUSED : ORTHO_EXACT) : tri;
-    ctx->info[6] = (use_simple_only ? 0 : 1) | ((int)global_hist << 2) | (box_type << 4) | (form << 8) | ((int)split << 12) | ((int)big << 13) | ((int64_t)tj << 16);
+    const bool skip_used = skip && !big && !split && !global_hist && !use_simple_only;
+    ctx->info[6] = (use_simple_only ? 0 : 1) | ((int)global_hist << 2) | (box_type << 4) | (form << 8) | ((int)split << 12) | ((int)big << 13) |
+                   ((int)skip_used << 14) | ((int64_t)tj << 16);
     ctx->info[7] = (int64_t)wt.padded_pairs;
     return CDH_OK;
 }
@@ -562,6 +613,79 @@ extern "C" int cdh_histograms_host(cdh_ctx* ctx, const void* coords, int32_t n_f
     ctx->flags = saved_flags;
     if (rc != CDH_OK) return rc;
     CDH_CUDA(cudaMemcpyAsync(out, ctx->d_io_out, obytes, cudaMemcpyDeviceToHost, stream));                      // one D2H copy
+    CDH_CUDA(cudaStreamSynchronize(stream));
+    return CDH_OK;
+}
+
+#ifndef CDH_STREAM_CHUNK_PAIRS
+#define CDH_STREAM_CHUNK_PAIRS 8.0e9    // automatic chunk: the fewest frames with this many pairs (several ms of tile kernel,
+                                        // so the per-call cost -- tables, zeroing, the tail of the wave -- stays around 1 %)
+#endif
+#ifndef CDH_STREAM_CHUNK_BYTES
+#define CDH_STREAM_CHUNK_BYTES (1ull << 30)  // and at most this many coordinate bytes per chunk buffer
+#endif
+
+extern "C" int cdh_histograms_stream(cdh_ctx* ctx, const void* coords, int32_t n_frames, const int32_t* off,
+                                     int32_t n_species, int32_t box_type, const double* box, int32_t n_boxes,
+                                     double r_max, int32_t n_bins, int32_t precision, int32_t frames_per_chunk,
+                                     void* stream_, uint64_t* out) {
+    if (!ctx || frames_per_chunk < 0) return CDH_ERR_INVALID_ARG;
+    int rc = validate(coords, n_frames, off, n_species, box_type, box, n_boxes, r_max, n_bins, precision, out);
+    if (rc != CDH_OK) return rc;
+    cudaStream_t stream = (cudaStream_t)stream_;
+    DeviceGuard guard(ctx->device);
+    if (!guard.ok) return cuda_fail(ctx, cudaGetLastError(), "cudaSetDevice");
+    const size_t fbytes = (size_t)off[n_species] * 3 * (precision == CDH_F64 ? sizeof(double) : sizeof(float));
+    const size_t obytes = (size_t)(n_species * (n_species + 1) / 2) * (size_t)n_bins * sizeof(uint64_t);
+    int64_t fpc = frames_per_chunk;
+    if (fpc == 0) {
+        const double pairs = frame_pairs(off, n_species);
+        fpc = pairs > 0.0 ? (int64_t)std::ceil(CDH_STREAM_CHUNK_PAIRS / pairs) : n_frames;
+        if (fbytes > 0 && (uint64_t)fpc * fbytes > CDH_STREAM_CHUNK_BYTES) fpc = (int64_t)(CDH_STREAM_CHUNK_BYTES / fbytes);
+    }
+    if (fpc < 1) fpc = 1;
+    if (fpc > n_frames) fpc = n_frames;
+    if (!ctx->copy_stream) {
+        CDH_CUDA(cudaStreamCreateWithFlags(&ctx->copy_stream, cudaStreamNonBlocking));
+        for (int k = 0; k < 2; ++k) {
+            CDH_CUDA(cudaEventCreateWithFlags(&ctx->copied[k], cudaEventDisableTiming));
+            CDH_CUDA(cudaEventCreateWithFlags(&ctx->consumed[k], cudaEventDisableTiming));
+        }
+    }
+    const size_t chunk_bytes = (size_t)fpc * fbytes;
+    const int64_t n_chunks = ((int64_t)n_frames + fpc - 1) / fpc;
+    for (int k = 0; k < (n_chunks > 1 ? 2 : 1); ++k)
+        if ((rc = grow(ctx, &ctx->d_chunk[k], &ctx->chunk_bytes[k], chunk_bytes > 0 ? chunk_bytes : 16, false)) != CDH_OK) return rc;
+    if ((rc = grow(ctx, &ctx->d_io_out, &ctx->io_out_bytes, obytes, false)) != CDH_OK) return rc;
+    // the buffers may still be read by work a caller enqueued on `stream` before this call (an earlier call of this entry
+    // point ends synchronised, so in practice this orders nothing): the first copies wait for the stream's present tail
+    CDH_CUDA(cudaEventRecord(ctx->consumed[0], stream));
+    CDH_CUDA(cudaEventRecord(ctx->consumed[1], stream));
+    const uint32_t saved_flags = ctx->flags;
+    for (int64_t c = 0; c < n_chunks && rc == CDH_OK; ++c) {
+        const int k = (int)(c & 1);
+        const int64_t f0 = c * fpc;
+        const int32_t nf = (int32_t)((int64_t)n_frames - f0 < fpc ? (int64_t)n_frames - f0 : fpc);
+        cudaError_t e = cudaStreamWaitEvent(ctx->copy_stream, ctx->consumed[k], 0);      // buffer k is free again
+        if (e == cudaSuccess && fbytes)
+            e = cudaMemcpyAsync(ctx->d_chunk[k], (const char*)coords + (size_t)f0 * fbytes, (size_t)nf * fbytes,
+                                cudaMemcpyHostToDevice, ctx->copy_stream);               // each frame is copied once
+        if (e == cudaSuccess) e = cudaEventRecord(ctx->copied[k], ctx->copy_stream);
+        if (e == cudaSuccess) e = cudaStreamWaitEvent(stream, ctx->copied[k], 0);
+        if (e != cudaSuccess) { rc = cuda_fail(ctx, e, "cdh_histograms_stream: copy pipeline"); break; }
+        ctx->flags = c == 0 ? (saved_flags & ~CDH_FLAG_ACCUMULATE) : (saved_flags | CDH_FLAG_ACCUMULATE);
+        rc = cdh_histograms(ctx, ctx->d_chunk[k], nf, off, n_species, box_type,
+                            (box && n_boxes > 1) ? box + (size_t)f0 * 9 : box, n_boxes > 1 ? nf : n_boxes,
+                            r_max, n_bins, precision, stream_, (uint64_t*)ctx->d_io_out);
+        if (rc == CDH_OK && (e = cudaEventRecord(ctx->consumed[k], stream)) != cudaSuccess)
+            rc = cuda_fail(ctx, e, "cudaEventRecord");
+    }
+    ctx->flags = saved_flags;
+    if (rc != CDH_OK) {                     // leave nothing in flight that still reads the caller's buffer
+        cudaStreamSynchronize(ctx->copy_stream); cudaStreamSynchronize(stream); cudaGetLastError();
+        return rc;
+    }
+    CDH_CUDA(cudaMemcpyAsync(out, ctx->d_io_out, obytes, cudaMemcpyDeviceToHost, stream));
     CDH_CUDA(cudaStreamSynchronize(stream));
     return CDH_OK;
 }

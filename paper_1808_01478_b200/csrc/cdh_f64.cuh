@@ -165,7 +165,7 @@ __device__ __forceinline__ void bin_f64(double d2, double rmax, double scale, ui
 }
 
 // ---- K1 for doubles: same schedule, stages and flush rule as tile_kernel (cdh_tile.cuh) ------------
-template <int BOX, int T, int MINB, bool PBOX, int MODE>
+template <int BOX, int T, int MINB, bool PBOX, int MODE, bool SKIP = false>     // SKIP: as in cdh_tile.cuh
 __global__ void __launch_bounds__(T, MINB) tile_kernel_f64(const TileParams64 P) {
     extern __shared__ __align__(128) unsigned char smem[];
     constexpr int TI = T * kR;
@@ -240,6 +240,8 @@ __global__ void __launch_bounds__(T, MINB) tile_kernel_f64(const TileParams64 P)
         { const double2 a = __ldg(gi + 2), b = __ldg(gi + 3); yi[0] = a.x; yi[1] = a.y; yi[2] = b.x; yi[3] = b.y; }
         { const double2 a = __ldg(gi + 4), b = __ldg(gi + 5); zi[0] = a.x; zi[1] = a.y; zi[2] = b.x; zi[3] = b.y; }
         const uint32_t ig = i0 + 4u * tid;
+        const uint32_t ig_warp = i0 + 4u * ((uint32_t)tid & ~31u);   // first i-particle of my warp
+        const bool warp_idle = ig_warp >= (uint32_t)seg.ni;          // my warp holds padding only
 
         const bool masked = seg.same && (j0 < i0 + TI);
         const uint32_t n_stage = (j1 - j0 + kStageParticles - 1) / kStageParticles;
@@ -268,12 +270,13 @@ __global__ void __launch_bounds__(T, MINB) tile_kernel_f64(const TileParams64 P)
             mbar_wait(bar_addr + 8 * b, (stage_cnt >> 1) & 1u);
             const double2* sj = reinterpret_cast<const double2*>(stage0 + b * (kStageBytes64 / 8));
             const uint32_t jbase = j0 + s * kStageParticles;
-            const uint32_t n_grp = (min(j1 - jbase, (uint32_t)kStageParticles) + 3u) >> 2;
+            const uint32_t n_grp = (SKIP && warp_idle) ? 0u : (min(j1 - jbase, (uint32_t)kStageParticles) + 3u) >> 2;
             const bool stage_masked = masked && (jbase < i0 + TI);
-            auto body = [&](auto masked_c) {
+            // j-groups wholly below the diagonal for every lane of the warp are skipped, as is a padding-only warp
+            auto body = [&](auto masked_c, const uint32_t g_begin) {
                 constexpr bool MASKED = decltype(masked_c)::value;
 #pragma unroll 1
-                for (uint32_t g = 0; g < n_grp; ++g) {
+                for (uint32_t g = g_begin; g < n_grp; ++g) {
                     const uint32_t jg = jbase + 4u * g;
 #pragma unroll
                     for (int h = 0; h < 2; ++h) {                   // two j-particles at a time (register pressure)
@@ -292,7 +295,8 @@ __global__ void __launch_bounds__(T, MINB) tile_kernel_f64(const TileParams64 P)
                     }
                 }
             };
-            if (stage_masked) body(std::true_type{}); else body(std::false_type{});
+            if (stage_masked) body(std::true_type{}, (SKIP && ig_warp > jbase) ? min(n_grp, (ig_warp - jbase) >> 2) : 0u);
+            else body(std::false_type{}, 0u);
             __syncthreads();
             ++stage_cnt;
         }

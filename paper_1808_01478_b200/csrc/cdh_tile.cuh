@@ -16,6 +16,7 @@
 #define CDH_GUNROLL 1      // j-groups unrolled in the inner loop (2 was measured: cfg2 -0.4 %, cfg5 -1.6 %, cfg3 +1.4 %)
 #endif
 
+
 namespace cdh {
 
 constexpr int kGUnroll = CDH_GUNROLL;
@@ -27,7 +28,11 @@ __host__ __device__ constexpr int tile_smem_bytes(int smem_bins) {
     return kSmemHeader + 2 * kStageBytes + sizeof(BoxConst) + 16 + 4 * (smem_bins + 2);   // + Q3 slot + trash slot
 }
 
-template <int BOX, int TRI, int T, int VAR, int MODE, int MINB>
+// SKIP: a warp skips the j-groups that lie below the diagonal for all of its lanes, and every group if it holds only
+// padding i-particles (ragged last i-tile).  For frames of small species (a few i-tiles each) this is up to 44 % of a
+// diagonal block and half of a ragged tile; the host takes these variants only then (cdh_api.cu), because the warp-dependent
+// trip count costs the large-problem kernels 2-5 % (measured: config 2 1258 -> 1221, config 5 1914 -> 1816 Gpairs/s).
+template <int BOX, int TRI, int T, int VAR, int MODE, int MINB, bool SKIP = false>
 __global__ void __launch_bounds__(T, MINB) tile_kernel(const TileParams P) {
     extern __shared__ __align__(128) unsigned char smem[];
     constexpr int TI = T * kR;
@@ -118,6 +123,8 @@ __global__ void __launch_bounds__(T, MINB) tile_kernel(const TileParams P) {
         const float4 XI = __ldg(gi), YI = __ldg(gi + 1), ZI = __ldg(gi + 2);
         const float xi[4] = {XI.x, XI.y, XI.z, XI.w}, yi[4] = {YI.x, YI.y, YI.z, YI.w}, zi[4] = {ZI.x, ZI.y, ZI.z, ZI.w};
         const uint32_t ig = i0 + 4u * tid;          // index of my first i-particle inside the species
+        const uint32_t ig_warp = i0 + 4u * ((uint32_t)tid & ~31u);   // first i-particle of my warp (128 consecutive ones)
+        const bool warp_idle = ig_warp >= (uint32_t)seg.ni;          // ragged last i-tile: my warp holds padding only
 
         const bool masked = seg.same && (j0 < i0 + TI);       // some j <= some i: test j > i per pair
         const uint32_t n_stage = (j1 - j0 + kStageParticles - 1) / kStageParticles;
@@ -153,12 +160,14 @@ __global__ void __launch_bounds__(T, MINB) tile_kernel(const TileParams P) {
             mbar_wait(bar_addr + 8 * b, (stage_cnt >> 1) & 1u);
             const float4* sj = reinterpret_cast<const float4*>(stage0 + b * (kStageBytes / 4));
             const uint32_t jbase = j0 + s * kStageParticles;                   // species index of the stage's first j
-            const uint32_t n_grp = (min(j1 - jbase, (uint32_t)kStageParticles) + 3u) >> 2;
+            const uint32_t n_grp = (SKIP && warp_idle) ? 0u : (min(j1 - jbase, (uint32_t)kStageParticles) + 3u) >> 2;
 
-            auto body = [&](auto masked_c) {
+            // only stages that touch the diagonal band need the mask
+            const bool stage_masked = masked && (jbase < i0 + TI);
+            auto body = [&](auto masked_c, const uint32_t g_begin) {
                 constexpr bool MASKED = decltype(masked_c)::value;
 #pragma unroll kGUnroll
-                for (uint32_t g = 0; g < n_grp; ++g) {
+                for (uint32_t g = g_begin; g < n_grp; ++g) {
                     const float4 XJ = sj[3 * g], YJ = sj[3 * g + 1], ZJ = sj[3 * g + 2];
                     const uint32_t jg = jbase + 4u * g;
                     if constexpr (VAR != VAR_FAST) {
@@ -226,9 +235,8 @@ __global__ void __launch_bounds__(T, MINB) tile_kernel(const TileParams P) {
                     }
                 }
             };
-            // only stages that touch the diagonal band need the mask
-            const bool stage_masked = masked && (jbase < i0 + TI);
-            if (stage_masked) body(std::true_type{}); else body(std::false_type{});
+            if (stage_masked) body(std::true_type{}, (SKIP && ig_warp > jbase) ? min(n_grp, (ig_warp - jbase) >> 2) : 0u);
+            else body(std::false_type{}, 0u);
 
             __syncthreads();          // everyone is done with buffer b before it is refilled
             ++stage_cnt;

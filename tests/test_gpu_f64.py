@@ -163,3 +163,18 @@ def test_f64_wide_histogram_global_and_split():
     q = inputs.reduced_config(3)
     c, info = gpu64(q, cdh.FLAG_GLOBAL_HIST)
     same(c, oracle64(q), "f64 triclinic, forced global histogram")
+
+
+@pytest.mark.parametrize("box_type", [inputs.BOX_NONE, inputs.BOX_ORTHO, inputs.BOX_TRICLINIC])
+def test_f64_small_species_take_the_skip_variants(box_type):
+    box = {inputs.BOX_NONE: None, inputs.BOX_ORTHO: np.diag([5.0, 6.0, 7.0]),
+           inputs.BOX_TRICLINIC: np.array([[6.0, 0.0, 0.0], [1.0, 5.5, 0.0], [-0.5, 1.5, 5.0]])}[box_type]
+    for counts in ((130,), (1025, 2047), (300, 1100, 2100), (4096, 3)):
+        p = inputs.uniform_problem(sum(counts) + 1, counts, box_type, 1500, 2.2, box=box, n_frames=2)
+        got, info = gpu64(p)
+        assert info["skip"], f"{counts}: {info}"
+        same(got, oracle64(p), f"f64 skip variant, box_type {box_type}, species {counts}")
+    big = inputs.uniform_problem(9, (9000, 14000), box_type, 1500, 2.2, box=box)
+    got, info = gpu64(big)
+    assert not info["skip"], info
+    same(got, oracle64(big), f"f64 large species, box_type {box_type}")

@@ -412,3 +412,20 @@ def test_triclinic_pairs_on_the_half_cell_switch_points(r_max):
     for flags in (0, cdh.FLAG_NO_PRUNE, cdh.FLAG_SIMPLE_KERNEL):
         got, info = gpu_hist(p, flags)
         assert_same(got, want, f"flags {flags:#x} {info}")
+
+
+@pytest.mark.parametrize("box_type", [inputs.BOX_NONE, inputs.BOX_ORTHO, inputs.BOX_TRICLINIC])
+def test_small_species_take_the_skip_variants(box_type):
+    # species of a few i-tiles each: the launch plan takes the kernels whose warps skip the j-groups below the diagonal
+    # and the padding-only warps of a ragged i-tile (info["skip"]); same integers as the oracle, and as the plain kernel
+    box = {inputs.BOX_NONE: None, inputs.BOX_ORTHO: np.diag([5.0, 6.0, 7.0]),
+           inputs.BOX_TRICLINIC: np.array([[6.0, 0.0, 0.0], [1.0, 5.5, 0.0], [-0.5, 1.5, 5.0]])}[box_type]
+    for counts in ((130,), (1024,), (1025, 2047), (300, 1100, 2100), (4096, 3), (2500, 2500)):
+        p = inputs.uniform_problem(sum(counts), counts, box_type, 1500, 2.2, box=box, n_frames=2)
+        got, info = gpu_hist(p)
+        assert info["skip"], f"{counts}: {info}"
+        assert_same(got, oracle_hist(p), f"skip variant, box_type {box_type}, species {counts}")
+    big = inputs.uniform_problem(7, (9000, 14000), box_type, 1500, 2.2, box=box)
+    got, info = gpu_hist(big)
+    assert not info["skip"], info
+    assert_same(got, oracle_hist(big), f"large species, box_type {box_type}")

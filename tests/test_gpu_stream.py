@@ -1,0 +1,103 @@
+"""-m gpu: cdh_histograms_stream (include/cdh.h) -- a host trajectory fed chunk by chunk with the copy of one chunk
+overlapping the kernels of the previous one -- against the oracle, bin for bin, for every chunking.
+
+The result is a sum of integers (Eq. 2), so it may not depend on frames_per_chunk, on whether the host
+buffer is pageable or page-locked, or on the precision path's own staging.
+"""
+import numpy as np
+import pytest
+
+import paper_1808_01478_b200 as cdh
+from paper_1808_01478_b200 import inputs
+from oracle import oracle as cdh_oracle
+
+torch = pytest.importorskip("torch")
+pytestmark = pytest.mark.gpu
+
+
+def _need_gpu():
+    if not torch.cuda.is_available():
+        pytest.skip("no CUDA device")
+
+
+def oracle_hist(p, precision="f32"):
+    c = p.coords.astype(np.float64) if precision == "f64" else p.coords
+    return cdh_oracle.histograms(c, p.species_offsets, p.box_type, p.box, p.r_max, p.n_bins, precision=precision)
+
+
+def same(got, want, what):
+    if not np.array_equal(got, want):
+        d = got.astype(np.int64) - want.astype(np.int64)
+        raise AssertionError(f"{what}: {np.count_nonzero(d)} bins differ, L1 = {int(np.abs(d).sum())}, "
+                             f"sums {int(got.sum())} / {int(want.sum())}")
+
+
+def trajectory(n_frames=7):
+    return inputs.config4(n_frames=n_frames, counts=(600, 1900), n_bins=3000)
+
+
+@pytest.mark.parametrize("fpc", [0, 1, 2, 3, 7, 100])
+def test_every_chunking_gives_the_oracle_histograms(fpc):
+    _need_gpu()
+    p = trajectory()
+    want = oracle_hist(p)
+    with cdh.Context(0) as ctx:
+        got = ctx.cdh_histograms_stream(p.coords, p.species_offsets, p.box_type, p.box, p.r_max, p.n_bins,
+                                        frames_per_chunk=fpc)
+        same(got, want, f"pageable host buffer, {fpc} frames per chunk")
+        pinned = torch.from_numpy(p.coords).pin_memory()
+        s = torch.cuda.Stream()
+        got = ctx.cdh_histograms_stream(pinned, p.species_offsets, p.box_type, p.box, p.r_max, p.n_bins,
+                                        frames_per_chunk=fpc, stream=s)
+        same(got, want, f"page-locked host buffer on a side stream, {fpc} frames per chunk")
+        # the one-shot host entry on the same context afterwards (shared scratch) still agrees
+        same(ctx.cdh_histograms_host(p.coords, p.species_offsets, p.box_type, p.box, p.r_max, p.n_bins), want, "one shot")
+
+
+def test_per_frame_boxes_follow_their_chunk():
+    _need_gpu()
+    g = np.random.Generator(np.random.PCG64(34))
+    f, n = 5, 1300
+    boxes = np.stack([np.array([[7.0 + k, 0, 0], [1.0, 6.5, 0], [0.5 * k, -1.0, 8.0 - k]]) for k in range(f)])
+    coords = np.stack([(g.random((n, 3)) @ boxes[k]).astype(np.float32) for k in range(f)])
+    p = inputs.Problem("tri_per_frame_stream", coords, np.array([0, 300, n], dtype=np.int32), inputs.BOX_TRICLINIC,
+                       boxes.reshape(f, 9), 2.4, 999)
+    want = oracle_hist(p)
+    with cdh.Context(0) as ctx:
+        for fpc in (1, 2, 5):
+            got = ctx.cdh_histograms_stream(p.coords, p.species_offsets, p.box_type, p.box, p.r_max, p.n_bins,
+                                            frames_per_chunk=fpc)
+            same(got, want, f"per-frame triclinic boxes, {fpc} frames per chunk")
+
+
+def test_double_precision_trajectory():
+    _need_gpu()
+    p = trajectory(4)
+    want = oracle_hist(p, "f64")
+    with cdh.Context(0) as ctx:
+        got = ctx.cdh_histograms_stream(p.coords.astype(np.float64), p.species_offsets, p.box_type, p.box, p.r_max,
+                                        p.n_bins, precision=cdh.F64, frames_per_chunk=3)
+    same(got, want, "f64, chunks of 3 + 1 frames")
+
+
+def test_accumulate_context_and_repeated_calls_do_not_leak_into_the_result():
+    _need_gpu()
+    p = trajectory(3)
+    want = oracle_hist(p)
+    with cdh.Context(0, cdh.FLAG_ACCUMULATE) as ctx:            # the flag is for cdh_histograms only: overwritten here
+        for _ in range(3):
+            got = ctx.cdh_histograms_stream(p.coords, p.species_offsets, p.box_type, p.box, p.r_max, p.n_bins,
+                                            frames_per_chunk=2)
+            same(got, want, "repeated call")
+
+
+def test_invalid_arguments_are_refused_before_anything_runs():
+    _need_gpu()
+    p = trajectory(2)
+    with cdh.Context(0) as ctx:
+        with pytest.raises(cdh.CdhError) as e:
+            ctx.cdh_histograms_stream(p.coords, p.species_offsets, p.box_type, p.box, p.r_max, p.n_bins,
+                                      frames_per_chunk=-1)
+        assert e.value.code == -1            # CDH_ERR_INVALID_ARG
+        with pytest.raises(cdh.CdhError):
+            ctx.cdh_histograms_stream(p.coords, p.species_offsets, p.box_type, p.box, -1.0, p.n_bins)
