@@ -126,7 +126,7 @@ int cdh_histograms_host(cdh_ctx *ctx, const void *coords, int32_t n_frames,
  *
  *  coords            HOST pointer, [n_frames][n_total][3]; page-locked memory is needed for the copies to overlap
  *                    (pageable memory works, the copies then pass through the driver's staging buffer).
- *  frames_per_chunk  >= 1, or 0 = automatic (the fewest frames with 8e9 pairs, at most 1 GiB of coordinates).
+ *  frames_per_chunk  >= 1, or 0 = automatic (the fewest frames with 3e10 pairs, at most 1 GiB of coordinates).
  *  box, n_boxes      as cdh_histograms; with n_boxes == n_frames chunk c uses its own frames' boxes.
  *  out               HOST pointer, uint64 [n_hist][n_bins], overwritten.
  * The result is independent of frames_per_chunk (integer sums).  cdh_last_call_info describes the last chunk.

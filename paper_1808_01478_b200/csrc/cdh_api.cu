@@ -618,8 +618,9 @@ extern "C" int cdh_histograms_host(cdh_ctx* ctx, const void* coords, int32_t n_f
 }
 
 #ifndef CDH_STREAM_CHUNK_PAIRS
-#define CDH_STREAM_CHUNK_PAIRS 8.0e9    // automatic chunk: the fewest frames with this many pairs (several ms of tile kernel,
-                                        // so the per-call cost -- tables, zeroing, the tail of the wave -- stays around 1 %)
+#define CDH_STREAM_CHUNK_PAIRS 3.0e10   // automatic chunk: the fewest frames with this many pairs (about 25 ms of tile kernel: the
+                                        // 0.1 ms a chunk costs -- tables, zeroing, the tail of its wave -- stays below 0.5 %;
+                                        // measured on config 4: 7-frame chunks of 6 ms were 1.3 % slower than one call)
 #endif
 #ifndef CDH_STREAM_CHUNK_BYTES
 #define CDH_STREAM_CHUNK_BYTES (1ull << 30)  // and at most this many coordinate bytes per chunk buffer
