@@ -80,14 +80,14 @@ static double frame_pairs(const int32_t* off, int32_t n_species) {
 #define CDH_SKIP_EFFICIENCY 0.9   // the SKIP variants (cdh_tile.cuh) are taken when fewer than this share of the pair slots the
                                   // 1024-particle i-tiles walk are pairs of the problem
 #endif
-// Small species: the share of the walked pair slots (1024-particle i-tiles: full diagonal blocks, padded last tiles) that are
-// pairs of the problem decides whether the SKIP variants of the 256-thread kernels pay.
+// Small species: the share of the walked pair slots (1024-particle i-tiles: whole stages on the diagonal, padded last tiles)
+// that are pairs of the problem decides whether the SKIP variants of the 256-thread kernels pay.
 static bool small_species(const int32_t* off, int32_t n_species) {
     const double ti256 = 256.0 * kR;
     double walked = 0.0;
-    for (int p = 0; p < n_species; ++p) {
-        const double tiles = std::ceil((double)(off[p + 1] - off[p]) / ti256);
-        walked += 0.5 * tiles * (tiles + 1.0) * ti256 * ti256;
+    for (int p = 0; p < n_species; ++p) {                       // the count build_tables makes (WorkTables::padded_pairs)
+        const double np_ = (double)(off[p + 1] - off[p]), tiles = std::ceil(np_ / ti256);
+        walked += ti256 * (tiles * np_ - ti256 * 0.5 * tiles * (tiles - 1.0));          // i-tile t walks j from t * 1024 to n_p
         for (int q = p + 1; q < n_species; ++q) walked += tiles * ti256 * (double)(off[q + 1] - off[q]);
     }
     return walked > 0.0 && frame_pairs(off, n_species) < CDH_SKIP_EFFICIENCY * walked;

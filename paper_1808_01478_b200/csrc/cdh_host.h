@@ -216,7 +216,9 @@ inline void build_tables(int32_t n_frames, const int32_t* off, int32_t n_species
                         r.jc0 = (p == q) ? i0 / tj : 0u;
                         w->rows.push_back(r);
                         w->n_items += n_jc - r.jc0;
-                        w->padded_pairs += (uint64_t)(n_jc - r.jc0) * ti * tj;
+                        // the kernel starts at the first 256-particle stage that reaches the diagonal (i0 is a multiple of
+                        // the stage) and walks whole j-groups of 4 up to nj
+                        w->padded_pairs += (uint64_t)ti * ((((uint32_t)nj + 3u) & ~3u) - ((p == q) ? i0 : 0u));
                     }
                 }
             }

@@ -425,6 +425,10 @@ def test_small_species_take_the_skip_variants(box_type):
         got, info = gpu_hist(p)
         assert info["skip"], f"{counts}: {info}"
         assert_same(got, oracle_hist(p), f"skip variant, box_type {box_type}, species {counts}")
+        # info[7]: the pair slots the 1024-particle i-tiles are scheduled to walk: at least the pairs, at most full tiles
+        tiles = [-(-c // 1024) for c in counts]
+        full = p.n_frames * sum(1024 * t * sum(c + 3 for c in counts[k:]) for k, t in enumerate(tiles))
+        assert p.evaluated_pairs <= info["padded_pairs"] <= full, (p.evaluated_pairs, info["padded_pairs"], full)
     big = inputs.uniform_problem(7, (9000, 14000), box_type, 1500, 2.2, box=box)
     got, info = gpu_hist(big)
     assert not info["skip"], info
