@@ -77,8 +77,9 @@ static double frame_pairs(const int32_t* off, int32_t n_species) {
 }
 
 #ifndef CDH_SKIP_EFFICIENCY
-#define CDH_SKIP_EFFICIENCY 0.9   // the SKIP variants (cdh_tile.cuh) are taken when fewer than this share of the pair slots the
-                                  // 1024-particle i-tiles walk are pairs of the problem
+#define CDH_SKIP_EFFICIENCY 0.95  // the SKIP variants (cdh_tile.cuh) are taken when fewer than this share of the pair slots the
+                                  // 1024-particle i-tiles walk are pairs of the problem (measured break-even, one species per
+                                  // frame: 16,384 particles, share 0.94: +0.7 %; 24,000 particles, share 0.96: -0.4 %)
 #endif
 // Small species: the share of the walked pair slots (1024-particle i-tiles: whole stages on the diagonal, padded last tiles)
 // that are pairs of the problem decides whether the SKIP variants of the 256-thread kernels pay.

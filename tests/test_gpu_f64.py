@@ -174,7 +174,7 @@ def test_f64_small_species_take_the_skip_variants(box_type):
         got, info = gpu64(p)
         assert info["skip"], f"{counts}: {info}"
         same(got, oracle64(p), f"f64 skip variant, box_type {box_type}, species {counts}")
-    big = inputs.uniform_problem(9, (9000, 14000), box_type, 1500, 2.2, box=box)
+    big = inputs.uniform_problem(9, (16000, 24000), box_type, 1500, 2.2, box=box)
     got, info = gpu64(big)
     assert not info["skip"], info
     same(got, oracle64(big), f"f64 large species, box_type {box_type}")

@@ -429,7 +429,7 @@ def test_small_species_take_the_skip_variants(box_type):
         tiles = [-(-c // 1024) for c in counts]
         full = p.n_frames * sum(1024 * t * sum(c + 3 for c in counts[k:]) for k, t in enumerate(tiles))
         assert p.evaluated_pairs <= info["padded_pairs"] <= full, (p.evaluated_pairs, info["padded_pairs"], full)
-    big = inputs.uniform_problem(7, (9000, 14000), box_type, 1500, 2.2, box=box)
+    big = inputs.uniform_problem(7, (16000, 24000), box_type, 1500, 2.2, box=box)
     got, info = gpu_hist(big)
     assert not info["skip"], info
     assert_same(got, oracle_hist(big), f"large species, box_type {box_type}")
