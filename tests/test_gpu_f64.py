@@ -105,6 +105,35 @@ def test_f64_config2_full_size():
     assert got.sum() / p.evaluated_pairs == pytest.approx(math.pi / 6, rel=2e-3)
 
 
+def test_f64_config3_full_size():
+    """Config 3 at full size in double, tied to the fp64 oracle as tests/test_gpu_fullsize.py does in float: the
+    (0,0) row outright, every row against the same kernels with the pruning off (27 shifts for every pair, the
+    oracle's own order of work), and the closed-form kept fraction pi/12 (V = d^3 sqrt(2)/2, r_max = d sqrt(2)/4)."""
+    p = inputs.config3()
+    got, info = gpu64(p)
+    assert info["sweeps"] == 1
+    a = inputs.Problem("cfg3_A", p.coords[:, :40000], np.array([0, 40000], dtype=np.int32), p.box_type, p.box, p.r_max, p.n_bins)
+    same(got[0:1], oracle64(a), "config 3 row (0,0) in double vs oracle")
+    full, _ = gpu64(p, cdh.FLAG_NO_PRUNE)
+    same(got, full, "config 3 in double: pruned vs 27-shift search everywhere")
+    assert got.sum() / p.evaluated_pairs == pytest.approx(math.pi / 12, rel=2e-3)
+
+
+def test_f64_config5_full_size():
+    """Config 5 at full size in double: every pair is binned, a species split adds up to the
+    one-species histogram, and the oracle computes the (A, A) block outright."""
+    p = inputs.config5()
+    got, info = gpu64(p)
+    assert info["sweeps"] == 1
+    assert int(got.sum()) == 499_999_500_000
+    n_a = 50_000
+    sp = inputs.Problem("cfg5_split", p.coords, np.array([0, n_a, p.n_total], dtype=np.int32), p.box_type, p.box, p.r_max, p.n_bins)
+    split, _ = gpu64(sp)
+    same(split.sum(axis=0, keepdims=True), got, "config 5 in double: (A,A) + (A,B) + (B,B) vs the one-species call")
+    a = inputs.Problem("cfg5_A", p.coords[:, :n_a], np.array([0, n_a], dtype=np.int32), p.box_type, p.box, p.r_max, p.n_bins)
+    same(split[0:1], oracle64(a), "config 5 block (A,A) in double vs oracle")
+
+
 def test_f64_sqrt_selftest_sample():
     if not torch.cuda.is_available():
         pytest.skip("no CUDA device")
