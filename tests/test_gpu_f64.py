@@ -119,6 +119,23 @@ def test_f64_config3_full_size():
     assert got.sum() / p.evaluated_pairs == pytest.approx(math.pi / 12, rel=2e-3)
 
 
+def test_f64_config4_full_size():
+    """Config 4 at full size in double: the 64-frame call equals the sum of 8-frame calls (Eq. 2) and the
+    oracle computes one of the chunks outright."""
+    p = inputs.config4()
+    got, _ = gpu64(p)
+    parts = np.zeros_like(got)
+    for f0 in range(0, 64, 8):
+        chunk = inputs.Problem(f"cfg4_{f0}", np.ascontiguousarray(p.coords[f0:f0 + 8]), p.species_offsets, p.box_type, p.box,
+                               p.r_max, p.n_bins)
+        h, _ = gpu64(chunk)
+        if f0 == 40:
+            same(h, oracle64(chunk), "config 4 frames 40..47 in double vs oracle")
+        parts += h
+    same(got, parts, "config 4 in double: 64 frames in one call vs the sum of 8-frame calls")
+    assert got.sum() / p.evaluated_pairs == pytest.approx(math.pi / 6, rel=2e-3)
+
+
 def test_f64_config5_full_size():
     """Config 5 at full size in double: every pair is binned, a species split adds up to the
     one-species histogram, and the oracle computes the (A, A) block outright."""
