@@ -62,3 +62,38 @@ def test_sample_problem_is_pure_slicing():
     s = bench.sample_problem(p, 0.25, 2)
     assert s.n_frames == 2 and s.species_counts() == [275, 1075] and s.n_bins == p.n_bins and s.r_max == p.r_max
     assert (s.coords[1, 275] == p.coords[1, 1100]).all()      # first particle of species 1
+
+
+def test_gpus_flag_starts_the_ranks_itself():
+    """`python bench.py --gpus 2` without torchrun must start two ranks (here: gloo on the CPU, no GPU work)."""
+    import json
+    import subprocess
+    env = {k: v for k, v in os.environ.items() if k not in ("RANK", "WORLD_SIZE", "LOCAL_RANK", "MASTER_ADDR", "MASTER_PORT")}
+    env["CUDA_VISIBLE_DEVICES"] = ""
+    r = subprocess.run([sys.executable, os.path.join(ROOT, "bench.py"), "--gpus", "2", "--rank-check"], env=env,
+                       capture_output=True, text=True, timeout=300)
+    assert r.returncode == 0, r.stderr[-2000:]
+    lines = [json.loads(s) for s in r.stdout.splitlines() if s.startswith("{")]
+    assert len(lines) == 1                                    # only rank 0 prints
+    assert lines[0]["n_gpus"] == 2 and lines[0]["max_ms"] == 11.0
+    assert lines[0]["value"] == pytest.approx(2 * 1e9 / 11e-3 / 1e9)
+
+
+def test_both_arms_print_the_same_config_object():
+    sys.path.insert(0, ROOT)
+    import bench
+    from paper_1808_01478_b200 import inputs
+    p = inputs.config1()
+    a = bench.config_block(p, bench.WORKLOADS[1], 1, (2, 3, 4, 5))
+    b = bench.config_block(p, bench.WORKLOADS[1], 1, bench.GATING_CONFIGS)
+    assert a == b and a["headline_config"] == 5 and a["configs_timed"] == [2, 3, 4, 5]
+
+
+def test_expected_wavefronts_of_uniform_bins():
+    sys.path.insert(0, ROOT)
+    import numpy as np
+    import bench
+    # 32 uniform draws over many bins: the expected maximum load of 32 balls in 32 bins, about 3.5
+    assert 3.4 < bench.expected_wavefronts(np.ones(50000), 1.0) < 3.65
+    # one bin only: every lane hits the same address, which the hardware merges into one wavefront
+    assert bench.expected_wavefronts(np.array([0.0, 5.0, 0.0]), 1.0) == 1.0
