@@ -7,7 +7,8 @@ imports nothing else of the package and never touches the CUDA library.
 
 Each file holds
     hist        uint64 [n_hist, n_bins]   the oracle's result (config 4: summed over the 64 frames, Eq. 2)
-    frame_hist  uint64 [n_frames, n_hist, n_bins]  (config 4 only: each frame by itself, so chunked calls can be checked)
+    chunk_hist  uint64 [n_frames / 8, n_hist, n_bins]  (config 4 only: the sum over each run of 8 consecutive frames, so that
+                chunked calls can be checked against the oracle too)
     sha_inputs  sha256 of coords bytes + species offsets + box + r_max + n_bins
     sha_oracle  sha256 of oracle/cdh_oracle.c
     seconds, threads  how long the oracle took here
@@ -44,6 +45,9 @@ _spec.loader.exec_module(inputs)
 from oracle import oracle as cdh_oracle  # noqa: E402
 
 
+CHUNK_FRAMES = 8
+
+
 def sha_inputs(p) -> str:
     h = hashlib.sha256()
     h.update(np.ascontiguousarray(p.coords).tobytes())
@@ -74,7 +78,8 @@ def make(config: int, precision: str) -> None:
                                               precision=precision)
             print(f"  cfg{config} {precision} frame {f + 1}/{p.n_frames}  {time.time() - t0:.0f} s", flush=True)
         hist = frames.sum(axis=0, dtype=np.uint64)
-        extra["frame_hist"] = frames
+        extra["chunk_hist"] = frames.reshape(p.n_frames // CHUNK_FRAMES, CHUNK_FRAMES, p.n_hist, p.n_bins).sum(axis=1, dtype=np.uint64)
+        extra["chunk_frames"] = CHUNK_FRAMES
     else:
         hist = cdh_oracle.problem_histograms(p, precision)
     dt = time.time() - t0

@@ -25,6 +25,12 @@ def gpu64(p, flags=0):
         return out.cpu().numpy().view(np.uint64), ctx.last_call_info()
 
 
+def golden64(config, p):
+    """The fp64 oracle's full-size histogram from tests/golden (written by make_fullsize.py, which calls only oracle/)."""
+    from test_gpu_fullsize import golden
+    return golden(config, p, "f64")
+
+
 def oracle64(p):
     return cdh_oracle.histograms(p.coords.astype(np.float64), p.species_offsets, p.box_type, p.box, p.r_max, p.n_bins,
                                  precision="f64")
@@ -112,8 +118,7 @@ def test_f64_config3_full_size():
     p = inputs.config3()
     got, info = gpu64(p)
     assert info["sweeps"] == 1
-    a = inputs.Problem("cfg3_A", p.coords[:, :40000], np.array([0, 40000], dtype=np.int32), p.box_type, p.box, p.r_max, p.n_bins)
-    same(got[0:1], oracle64(a), "config 3 row (0,0) in double vs oracle")
+    same(got, golden64(3, p)["hist"], "config 3 in double, all rows vs the oracle's full-size histogram")
     full, _ = gpu64(p, cdh.FLAG_NO_PRUNE)
     same(got, full, "config 3 in double: pruned vs 27-shift search everywhere")
     assert got.sum() / p.evaluated_pairs == pytest.approx(math.pi / 12, rel=2e-3)
@@ -124,13 +129,14 @@ def test_f64_config4_full_size():
     oracle computes one of the chunks outright."""
     p = inputs.config4()
     got, _ = gpu64(p)
+    g = golden64(4, p)
+    same(got, g["hist"], "config 4 in double, 64 frames in one call vs the oracle's full-size histogram")
     parts = np.zeros_like(got)
     for f0 in range(0, 64, 8):
         chunk = inputs.Problem(f"cfg4_{f0}", np.ascontiguousarray(p.coords[f0:f0 + 8]), p.species_offsets, p.box_type, p.box,
                                p.r_max, p.n_bins)
         h, _ = gpu64(chunk)
-        if f0 == 40:
-            same(h, oracle64(chunk), "config 4 frames 40..47 in double vs oracle")
+        same(h, g["chunk_hist"][f0 // 8], f"config 4 frames {f0}..{f0 + 7} in double vs the oracle's stored chunk sum")
         parts += h
     same(got, parts, "config 4 in double: 64 frames in one call vs the sum of 8-frame calls")
     assert got.sum() / p.evaluated_pairs == pytest.approx(math.pi / 6, rel=2e-3)
@@ -143,6 +149,7 @@ def test_f64_config5_full_size():
     got, info = gpu64(p)
     assert info["sweeps"] == 1
     assert int(got.sum()) == 499_999_500_000
+    same(got, golden64(5, p)["hist"], "config 5 in double, all 5e11 pairs vs the oracle's full-size histogram")
     n_a = 50_000
     sp = inputs.Problem("cfg5_split", p.coords, np.array([0, n_a, p.n_total], dtype=np.int32), p.box_type, p.box, p.r_max, p.n_bins)
     split, _ = gpu64(sp)

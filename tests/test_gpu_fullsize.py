@@ -1,14 +1,17 @@
 """-m gpu: the five BASELINE.json configs at FULL size, in the launch configuration bench.py times.
 
-Config 1 and 2: the whole result against the fp32 oracle.  Configs 3-5 are too large for the oracle to finish in
-seconds, so the full-size result is tied to it through exact decompositions of the integer histogram:
-  * a species split (extra offsets) turns one row into three rows that must add up to it, and the oracle computes
-    the (A, A) block outright;
-  * the sum over frames equals the sum of the per-chunk results, and the oracle computes one chunk outright;
-  * the remaining rows are compared with the plain cross-validation kernel (CDH_FLAG_SIMPLE_KERNEL, library
-    sqrtf / rintf / floorf, no pruning), itself pinned to the oracle on the oracle-sized blocks;
+Config 1 and 2: the whole result against the fp32 oracle, run here.  Configs 3, 4, 5: every bin of every row against
+the oracle's full-size histogram stored in tests/golden/cfg{3,4,5}_f32.npz (written once by tests/golden/make_fullsize.py,
+which calls only oracle/; SURVEY.md 8d "compute once, cache on disk"); the stored file carries the sha256 of the input
+bytes, re-checked here against the inputs the GPU is given.  On top of that, exact decompositions of the integer
+histogram (kept from round 1; they exercise other launch shapes):
+  * a species split (extra offsets) turns one row into three rows that must add up to it;
+  * the sum over frames equals the sum of the per-chunk results, each chunk against the oracle's stored chunk sum;
+  * the plain cross-validation kernel (CDH_FLAG_SIMPLE_KERNEL, library sqrtf / rintf / floorf, no pruning);
   * closed forms: total = N(N-1)/2 when r_max covers every pair, kept fraction = sphere / cell volume.
 """
+import hashlib
+import os
 import math
 
 import numpy as np
@@ -51,6 +54,22 @@ def ctx_simple():
         yield c
 
 
+GOLDEN = os.path.join(os.path.dirname(os.path.abspath(__file__)), "golden")
+
+
+def golden(config, p, precision="f32"):
+    """The oracle's stored full-size result; fails if the stored input hash is not that of ``p``."""
+    d = np.load(os.path.join(GOLDEN, f"cfg{config}_{precision}.npz"))
+    h = hashlib.sha256()
+    h.update(np.ascontiguousarray(p.coords).tobytes())
+    h.update(np.ascontiguousarray(p.species_offsets, dtype=np.int32).tobytes())
+    h.update(b"" if p.box is None else np.ascontiguousarray(p.box, dtype=np.float64).tobytes())
+    h.update(np.array([p.r_max], dtype=np.float64).tobytes())
+    h.update(np.array([p.n_bins, p.box_type], dtype=np.int64).tobytes())
+    assert h.hexdigest() == str(d["sha_inputs"]), "tests/golden was written for other inputs: rerun make_fullsize.py"
+    return d
+
+
 def with_offsets(p, offsets, name):
     return inputs.Problem(name, p.coords, np.asarray(offsets, dtype=np.int32), p.box_type, p.box, p.r_max, p.n_bins)
 
@@ -67,10 +86,8 @@ def test_config3_full(ctx, ctx_simple):
     got = run(ctx, p)
     info = ctx.last_call_info()
     assert info["fast"] and info["sweeps"] == 1
-    # (0,0) block outright against the oracle
-    a = inputs.Problem("cfg3_A", p.coords[:, :40000], np.array([0, 40000], dtype=np.int32), p.box_type, p.box, p.r_max, p.n_bins)
-    same(got[0:1], cdh_oracle.problem_histograms(a, "f32"), "config 3 row (0,0) vs oracle")
-    # all rows against the cross-validation kernel (27 shifts for every pair)
+    same(got, golden(3, p)["hist"], "config 3, all three rows vs the oracle's full-size histogram")
+    # and against the cross-validation kernel (27 shifts for every pair)
     same(got, run(ctx_simple, p), "config 3 vs plain kernel")
     assert got.sum() / p.evaluated_pairs == pytest.approx(math.pi / 12, rel=2e-3)     # V = d^3 sqrt(2)/2, r = d sqrt(2)/4
 
@@ -78,13 +95,14 @@ def test_config3_full(ctx, ctx_simple):
 def test_config4_full(ctx):
     p = inputs.config4()
     got = run(ctx, p)
+    g = golden(4, p)
+    same(got, g["hist"], "config 4, 64 frames in one call vs the oracle's full-size histogram")
     parts = np.zeros_like(got)
     for f0 in range(0, 64, 8):
         chunk = inputs.Problem(f"cfg4_{f0}", np.ascontiguousarray(p.coords[f0:f0 + 8]), p.species_offsets, p.box_type, p.box,
                                p.r_max, p.n_bins)
         h = run(ctx, chunk)
-        if f0 == 24:
-            same(h, cdh_oracle.problem_histograms(chunk, "f32"), "config 4 frames 24..31 vs oracle")
+        same(h, g["chunk_hist"][f0 // 8], f"config 4 frames {f0}..{f0 + 7} vs the oracle's stored chunk sum")
         parts += h
     same(got, parts, "config 4: 64 frames in one call vs the sum of 8-frame calls (Eq. 2)")
     assert got.sum() / p.evaluated_pairs == pytest.approx(math.pi / 6, rel=2e-3)
@@ -96,6 +114,7 @@ def test_config5_full(ctx):
     info = ctx.last_call_info()
     assert info["sweeps"] == 1 and info["fast"]
     assert int(got.sum()) == 499_999_500_000                     # P1: every pair is binned
+    same(got, golden(5, p)["hist"], "config 5, all 5e11 pairs vs the oracle's full-size histogram")
     n_a = 50_000
     split = run(ctx, with_offsets(p, [0, n_a, p.n_total], "cfg5_split"))
     same(split.sum(axis=0, keepdims=True), got, "config 5: (A,A) + (A,B) + (B,B) vs the one-species call")

@@ -414,3 +414,42 @@ def test_triclinic_with_diagonal_box_equals_ortho():
     b = oracle.histograms(p.coords, p.species_offsets, BOX_TRICLINIC, p.box, p.r_max, p.n_bins, precision="f64")
     assert np.abs(np.cumsum(a.astype(np.int64)) - np.cumsum(b.astype(np.int64))).max() <= 2
     assert abs(int(a.sum()) - int(b.sum())) <= 2
+
+
+# ---- the stored full-size oracle histograms (tests/golden/cfg{3,4,5}_{f32,f64}.npz, make_fullsize.py) ------------------
+@pytest.mark.parametrize("config,precision", [(c, p) for c in (3, 4, 5) for p in ("f32", "f64")])
+def test_fullsize_goldens_belong_to_these_inputs_and_this_oracle(config, precision):
+    """The files the GPU full-size tests compare against: written by the oracle source as it stands (sha256), for the
+    inputs the generators produce today (sha256), and consistent with what the mathematics fixes at full size --
+    the closed-form total where r_max covers every pair or the sphere/cell volume ratio of uniform
+    points, and the chunk sums adding up to the whole (Eq. 2)."""
+    import hashlib
+    import importlib.util
+    here = os.path.join(os.path.dirname(os.path.abspath(__file__)), "golden")
+    spec = importlib.util.spec_from_file_location("make_fullsize", os.path.join(here, "make_fullsize.py"))
+    mf = importlib.util.module_from_spec(spec)
+    spec.loader.exec_module(mf)
+    d = np.load(mf.path(config, precision))
+    assert str(d["sha_oracle"]) == mf.sha_oracle(), "oracle/cdh_oracle.c changed: rerun tests/golden/make_fullsize.py"
+    p = inputs.make_config(config)
+    assert str(d["sha_inputs"]) == mf.sha_inputs(p), "the seeded inputs changed: rerun tests/golden/make_fullsize.py"
+    h = d["hist"]
+    assert h.shape == (p.n_hist, p.n_bins) and h.dtype == np.uint64
+    kept = int(h.sum())
+    if config == 5:
+        assert kept == 1_000_000 * 999_999 // 2                         # every pair is within sqrt(3) of every other
+    else:
+        want = math.pi / 12 if config == 3 else math.pi / 6               # sphere of radius r_max / cell volume
+        assert kept / p.evaluated_pairs == pytest.approx(want, rel=2e-3)
+        per_row = h.sum(axis=1) / (np.array(p.pairs_per_hist(), dtype=np.float64) * p.n_frames)
+        assert np.allclose(per_row, want, rtol=1e-2)                      # every species pair separately
+    if config == 4:
+        assert d["chunk_hist"].shape == (8, p.n_hist, p.n_bins)
+        assert np.array_equal(d["chunk_hist"].sum(axis=0, dtype=np.uint64), h)
+    # ideal-gas shape of a uniform periodic system: counts grow like r^2 (compare two wide shells)
+    if config in (3, 4):
+        n = p.n_bins
+        a, b = h[:, n // 4: n // 4 + n // 8].sum(), h[:, n // 2: n // 2 + n // 8].sum()
+        r1, r2 = (n // 4, n // 4 + n // 8), (n // 2, n // 2 + n // 8)
+        want_ratio = (r2[1] ** 3 - r2[0] ** 3) / (r1[1] ** 3 - r1[0] ** 3)
+        assert b / a == pytest.approx(want_ratio, rel=5e-3)
