@@ -13,7 +13,10 @@ import sys
 _HERE = os.path.dirname(os.path.abspath(__file__))
 CSRC = os.path.join(_HERE, "csrc")
 LIB = os.path.join(_HERE, "libcdh.so")
-SOURCES = ["cdh_api.cu", "cdh_bench.cu"]
+# cdh_api.cu: the C ABI and host dispatch; cdh_k_*.cu: the tile-kernel instantiations, one translation unit per box
+# type so that they compile in parallel; cdh_bench.cu: the roofline microbenchmarks and self-tests.
+SOURCES = ["cdh_api.cu", "cdh_bench.cu", "cdh_k_none.cu", "cdh_k_ortho.cu", "cdh_k_tri.cu", "cdh_k_tri_wide.cu",
+           "cdh_k_simple.cu", "cdh_k_f64.cu"]
 INCLUDE = os.path.join(_HERE, "..", "include")
 
 
@@ -25,7 +28,8 @@ def deps():
 
 
 NVCC_FLAGS = ["-gencode", "arch=compute_100a,code=sm_100a", "-O3", "-lineinfo", "-std=c++17",
-              "-Xcompiler", "-fPIC,-ffp-contract=off,-fno-fast-math", "-shared", "-cudart", "static"]
+              "-Xcompiler", "-fPIC,-ffp-contract=off,-fno-fast-math"]
+LINK_FLAGS = ["-gencode", "arch=compute_100a,code=sm_100a", "-shared", "-cudart", "static"]
 
 
 def nvcc_path() -> str:
@@ -44,15 +48,31 @@ def is_stale() -> bool:
 
 def build(force: bool = False, verbose: bool = False, extra_flags=(), out: str = LIB) -> str:
     """Compile if the library is missing or older than a source; returns its path.  ``extra_flags`` / ``out``
-    build an experimental copy (e.g. ``-DCDH_MINB=3``) next to the product library."""
+    build an experimental copy (e.g. ``-DCDH_MINB=3``) next to the product library.  The translation units are
+    compiled concurrently (one nvcc process each), then linked into one shared object."""
     if force or out != LIB or is_stale():
-        tmp = out + f".tmp{os.getpid()}"
-        cmd = [nvcc_path(), *NVCC_FLAGS, *extra_flags, "-o", tmp, *[os.path.join(CSRC, s) for s in SOURCES]]
-        if verbose:
-            cmd.insert(1, "-Xptxas=-v")
-            print(" ".join(cmd), file=sys.stderr)
-        subprocess.run(cmd, check=True, cwd=CSRC)
-        os.replace(tmp, out)
+        import concurrent.futures
+        import tempfile
+        nvcc = nvcc_path()
+        with tempfile.TemporaryDirectory(prefix="cdh_build_") as tmpdir:
+            def compile_one(src):
+                obj = os.path.join(tmpdir, src.replace(".cu", ".o"))
+                cmd = [nvcc, *NVCC_FLAGS, *extra_flags, "-c", "-o", obj, os.path.join(CSRC, src)]
+                if verbose:
+                    cmd.insert(1, "-Xptxas=-v")
+                    print(" ".join(cmd), file=sys.stderr)
+                r = subprocess.run(cmd, cwd=CSRC, capture_output=True, text=True)
+                return src, obj, r
+            with concurrent.futures.ThreadPoolExecutor(max_workers=min(len(SOURCES), os.cpu_count() or 1)) as pool:
+                results = list(pool.map(compile_one, SOURCES))
+            for src, _obj, r in results:
+                if verbose or r.returncode != 0:
+                    sys.stderr.write(r.stdout + r.stderr)
+                if r.returncode != 0:
+                    raise subprocess.CalledProcessError(r.returncode, f"nvcc -c {src}")
+            tmp = out + f".tmp{os.getpid()}"
+            subprocess.run([nvcc, *LINK_FLAGS, "-o", tmp, *[obj for _s, obj, _r in results]], check=True, cwd=CSRC)
+            os.replace(tmp, out)
     return out
 
 

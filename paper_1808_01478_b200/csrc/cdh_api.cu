@@ -1,14 +1,49 @@
-// cdh_api.cu -- the C ABI of libcdh (include/cdh.h): context, validation, host dispatch.
-// All device work of a call is enqueued on the caller's stream; cdh_histograms never synchronises.
+// cdh_api.cu -- the C ABI of libcdh (include/cdh.h): context, validation, plans, host dispatch.
+//
+// A PLAN is everything of a call that depends on its arguments but not on the coordinate values: the box constants,
+// the padded layout, the work tables (uploaded once, into the plan's own device buffer), the kernel variants of the
+// launch plan with their shared-memory sizes and grids.  Plans are cached per context (cdh_ctx::plans, least recently
+// used out), so a trajectory fed frame by frame or chunk by chunk -- the paper's use case, PAPER.md:233, 338 -- pays the
+// host work and the table upload once; a call that hits the cache enqueues two memsets, the repack kernel and the tile
+// launches and touches no allocator and no event.  All device work of a call is enqueued on the caller's stream.
+#include <algorithm>
 #include <cstdio>
+#include <memory>
 #include <new>
 #include <string>
 #include "cdh_host.h"
-#include "cdh_tile.cuh"
+#include "cdh_math32.cuh"
 #include "cdh_f64.cuh"
 #include "cdh_rdf.cuh"
+#include "cdh_variants.h"
 
 using namespace cdh;
+
+namespace {
+
+struct Launch { Variant v; float lo, hi; };
+
+struct Plan {
+    std::vector<unsigned char> key;      // the arguments the plan was built from
+    uint64_t stamp = 0;                  // last use (LRU)
+    void* d_tables = nullptr;            // segs | rows | boxes | off | pad_off | row_seg | win_lo
+    cudaEvent_t uploaded = nullptr;      // the table upload (recorded on up_stream)
+    cudaStream_t up_stream = nullptr;
+    size_t pk_bytes = 0;                 // repacked coordinates the call needs
+    int precision = CDH_F32, box_type = 0, n_hist = 0, n_species = 0, n_frames = 0, n_boxes = 1, n_total = 0;
+    uint32_t n_bins = 0, frame_slots = 0, repack_blocks = 0, blocks_per_frame = 0;
+    size_t o_rows = 0, o_boxes = 0, o_off = 0, o_pad = 0, o_rowseg = 0, o_win = 0;
+    std::vector<Launch> launches;
+    int smem_bytes = 0, mode = MODE_SHARED;
+    uint32_t grid = 0, n_items = 0, n_rows = 0, tj = 0, smem_bins = 0, n_stages = 2;
+    double r_max = 0.0;
+    float rmax_f = 0.f, scale_f = 0.f;
+    uint32_t thr2_bits = 0;
+    BoxConst64 box0_64;                  // CDH_F64 PBOX variants
+    int64_t info[8] = {0, 0, 0, 0, 0, 0, 0, 0};
+};
+
+}  // namespace
 
 struct cdh_ctx {
     int device = 0;
@@ -16,12 +51,12 @@ struct cdh_ctx {
     int n_sm = 0;
     int max_smem_optin = 0;
     // device scratch, grown on demand, never shrunk
-    float* d_pk = nullptr;       size_t pk_bytes = 0;
-    void* d_tables = nullptr;    size_t tables_bytes = 0;     // segs | rows | boxes | off | pad_off
-    unsigned int* d_scalars = nullptr;                        // [0..2] work counters of the call's tile launches, [4..9] range keys (repack_kernel)
-    void* h_tables = nullptr;    size_t h_tables_bytes = 0;   // pinned staging for d_tables
+    void* d_pk = nullptr;        size_t pk_bytes = 0;         // repacked coordinates of the call in flight
+    unsigned int* d_scalars = nullptr;                        // [0..2] work counters of the call's tile launches, [4..10] range keys (repack_kernel)
+    void* h_tables = nullptr;    size_t h_tables_bytes = 0;   // pinned staging for a new plan's tables
     cudaEvent_t staged = nullptr;                             // h_tables may be rewritten once this has fired
     bool staged_pending = false;
+    void* d_small = nullptr;     size_t small_bytes = 0;      // cdh_rdf: densities
     void* d_io_coords = nullptr; size_t io_coords_bytes = 0;  // cdh_histograms_host staging
     void* d_io_out = nullptr;    size_t io_out_bytes = 0;
     // cdh_histograms_stream: two chunk buffers filled on a private copy stream while the other is being processed
@@ -30,11 +65,15 @@ struct cdh_ctx {
     cudaEvent_t copied[2] = {nullptr, nullptr}, consumed[2] = {nullptr, nullptr};
     cudaEvent_t* ev = nullptr;   // CDH_FLAG_TIME_KERNELS: ring of [CDH_TIMED_CALLS][4]: call begin, tile begin, tile end, call end
     uint64_t timed_calls = 0;
+    std::vector<std::unique_ptr<Plan>> plans;
+    uint64_t stamp = 0;
     std::string err;
     int64_t info[8] = {0, 0, 0, 0, 0, 0, 0, 0};
 };
 
 namespace {
+
+constexpr size_t kMaxPlans = 16;
 
 struct DeviceGuard {
     int prev = -1; bool ok;
@@ -49,10 +88,11 @@ int cuda_fail(cdh_ctx* c, cudaError_t e, const char* what) {
 #define CDH_CUDA(call)                                                       \
     do { cudaError_t e_ = (call); if (e_ != cudaSuccess) return cuda_fail(ctx, e_, #call); } while (0)
 
+// Grows a scratch buffer of the context.  A buffer that enqueued work may still read is not freed under it: the
+// device is synchronised first.  Happens only when a call needs more scratch than any call before it.
 int grow(cdh_ctx* ctx, void** p, size_t* have, size_t need, bool pinned_host) {
     if (need <= *have) return CDH_OK;
     if (*p) {
-        // a buffer still in use by enqueued work must not be freed under it
         cudaError_t e = cudaDeviceSynchronize();
         if (e != cudaSuccess) return cuda_fail(ctx, e, "cudaDeviceSynchronize");
         if (pinned_host) cudaFreeHost(*p); else cudaFree(*p);
@@ -66,7 +106,7 @@ int grow(cdh_ctx* ctx, void** p, size_t* have, size_t need, bool pinned_host) {
 }
 
 // Pairs one frame evaluates (all species pairs).
-static double frame_pairs(const int32_t* off, int32_t n_species) {
+double frame_pairs(const int32_t* off, int32_t n_species) {
     double tot = 0.0;
     for (int p = 0; p < n_species; ++p) {
         const double np_ = (double)(off[p + 1] - off[p]);
@@ -77,13 +117,13 @@ static double frame_pairs(const int32_t* off, int32_t n_species) {
 }
 
 #ifndef CDH_SKIP_EFFICIENCY
-#define CDH_SKIP_EFFICIENCY 0.95  // the SKIP variants (cdh_tile.cuh) are taken when fewer than this share of the pair slots the
+#define CDH_SKIP_EFFICIENCY 0.95  // the SKIP variants (cdh_sched.cuh) are taken when fewer than this share of the pair slots the
                                   // 1024-particle i-tiles walk are pairs of the problem (measured break-even, one species per
                                   // frame: 16,384 particles, share 0.94: +0.7 %; 24,000 particles, share 0.96: -0.4 %)
 #endif
 // Small species: the share of the walked pair slots (1024-particle i-tiles: whole stages on the diagonal, padded last tiles)
 // that are pairs of the problem decides whether the SKIP variants of the 256-thread kernels pay.
-static bool small_species(const int32_t* off, int32_t n_species) {
+bool small_species(const int32_t* off, int32_t n_species) {
     const double ti256 = 256.0 * kR;
     double walked = 0.0;
     for (int p = 0; p < n_species; ++p) {                       // the count build_tables makes (WorkTables::padded_pairs)
@@ -94,64 +134,24 @@ static bool small_species(const int32_t* off, int32_t n_species) {
     return walked > 0.0 && frame_pairs(off, n_species) < CDH_SKIP_EFFICIENCY * walked;
 }
 
-// ---- kernel table -----------------------------------------------------------------------------
-typedef void (*TileFn)(const TileParams);
-struct Variant { TileFn fn; int threads; };
-
-#ifndef CDH_GLOBAL_SWEEPS
-#define CDH_GLOBAL_SWEEPS 8   // shared-memory sweeps from which the global-histogram mode takes over (measured
-                              // break-even: 200,000 uniform points, 400,000 bins: 8 sweeps 200 vs global 221 Gpairs/s)
-#endif
-constexpr uint32_t kGlobalSweeps = CDH_GLOBAL_SWEEPS;
 #ifndef CDH_ITEMS_PER_CTA
 #define CDH_ITEMS_PER_CTA 64   // work items per resident CTA the j-chunk size is shrunk for (tail of the dynamic schedule)
 #endif
 constexpr uint64_t kItemsPerCta = CDH_ITEMS_PER_CTA;
-#ifndef CDH_MINB
-#define CDH_MINB 3      // resident CTAs per SM the 256-thread NONE / ORTHO fast variants are register-bounded for
-                        // (80 registers; measured +1.5 % over 2; the triclinic variants need 128 registers: 2)
+#ifndef CDH_STAGES
+#define CDH_STAGES 4           // stages of the TMA ring (cdh_sched.cuh) when the private histogram leaves the room; else 2
 #endif
-#ifndef CDH_BIG_T
-#define CDH_BIG_T 1024  // threads of the one-CTA-per-SM variants (32 warps/SM: config 5 +5 % over 512)
-#endif
-template <int BOX, int TRI, int MODE>
-Variant fast_variant(bool big, bool skip) {
-    if constexpr (MODE != MODE_GLOBAL)
-        if (big) return {tile_kernel<BOX, TRI, CDH_BIG_T, VAR_FAST, MODE, 1>, CDH_BIG_T};
-    if constexpr (MODE == MODE_SHARED)
-        if (skip) return {tile_kernel<BOX, TRI, 256, VAR_FAST, MODE, (BOX == BOX_TRI ? 2 : CDH_MINB), true>, 256};
-    return {tile_kernel<BOX, TRI, 256, VAR_FAST, MODE, (BOX == BOX_TRI ? 2 : CDH_MINB)>, 256};
+
+Variant fast_variant(int box_type, int form, int mode, int shape) {
+    if (box_type == CDH_BOX_NONE) return fast_variant_none(mode, shape);
+    if (box_type == CDH_BOX_ORTHO) return fast_variant_ortho(form, mode, shape);
+    return (form & TRI_WIDE) ? fast_variant_tri_wide(form, mode, shape) : fast_variant_tri(form, mode, shape);
 }
-template <int SPLIT>
-Variant pick_fast(int box_type, int tri, bool big, bool skip) {      // tri: TRI_* for TRICLINIC, ORTHO_* for ORTHO
-    if (box_type == CDH_BOX_NONE) return fast_variant<BOX_NONE, 0, SPLIT>(big, skip);
-    if (box_type == CDH_BOX_ORTHO)
-        return tri == ORTHO_FUSED ? fast_variant<BOX_ORTHO, ORTHO_FUSED, SPLIT>(big, skip)
-             : tri == ORTHO_EXACT ? fast_variant<BOX_ORTHO, ORTHO_EXACT, SPLIT>(big, skip) : fast_variant<BOX_ORTHO, ORTHO_PLAIN, SPLIT>(big, skip);
-    if (tri == TRI_UPPER_B01) return fast_variant<BOX_TRI, TRI_UPPER_B01, SPLIT>(big, skip);
-    if (tri == TRI_UPPER) return fast_variant<BOX_TRI, TRI_UPPER, SPLIT>(big, skip);
-    if (tri == (TRI_UPPER_B01 | TRI_WIDE)) return fast_variant<BOX_TRI, TRI_UPPER_B01 | TRI_WIDE, SPLIT>(big, skip);
-    if (tri == (TRI_UPPER | TRI_WIDE)) return fast_variant<BOX_TRI, TRI_UPPER | TRI_WIDE, SPLIT>(big, skip);
-    if (tri == (TRI_GENERAL | TRI_WIDE)) return fast_variant<BOX_TRI, TRI_GENERAL | TRI_WIDE, SPLIT>(big, skip);
-    return fast_variant<BOX_TRI, TRI_GENERAL, SPLIT>(big, skip);
-}
-template <int VAR>
-Variant simple_variant(int box_type, bool big) {
-    if (box_type == CDH_BOX_NONE)
-        return big ? Variant{tile_kernel<BOX_NONE, 0, CDH_BIG_T, VAR, MODE_SPLIT, 1>, CDH_BIG_T} : Variant{tile_kernel<BOX_NONE, 0, 256, VAR, MODE_SPLIT, 2>, 256};
-    if (box_type == CDH_BOX_ORTHO)
-        return big ? Variant{tile_kernel<BOX_ORTHO, 0, CDH_BIG_T, VAR, MODE_SPLIT, 1>, CDH_BIG_T} : Variant{tile_kernel<BOX_ORTHO, 0, 256, VAR, MODE_SPLIT, 2>, 256};
-    return big ? Variant{tile_kernel<BOX_TRI, 0, CDH_BIG_T, VAR, MODE_SPLIT, 1>, CDH_BIG_T} : Variant{tile_kernel<BOX_TRI, 0, 256, VAR, MODE_SPLIT, 2>, 256};
-}
-Variant simple_global(int box_type) {
-    if (box_type == CDH_BOX_NONE) return {tile_kernel<BOX_NONE, 0, 256, VAR_SIMPLE, MODE_GLOBAL, 2>, 256};
-    if (box_type == CDH_BOX_ORTHO) return {tile_kernel<BOX_ORTHO, 0, 256, VAR_SIMPLE, MODE_GLOBAL, 2>, 256};
-    return {tile_kernel<BOX_TRI, 0, 256, VAR_SIMPLE, MODE_GLOBAL, 2>, 256};
-}
-Variant pick_simple(int box_type, bool big, uint32_t flags) {
-    if (flags & CDH_FLAG_WARP_AGGREGATE) return simple_variant<VAR_SIMPLE_MATCH>(box_type, big);
-    if (flags & CDH_FLAG_NO_AGGREGATE) return simple_variant<VAR_SIMPLE_PLAIN>(box_type, big);
-    return simple_variant<VAR_SIMPLE>(box_type, big);
+
+inline size_t align256(size_t x) { return (x + 255) & ~(size_t)255; }
+
+int smem_fixed(int precision, int n_stages) {
+    return precision == CDH_F64 ? tile_smem_fixed<MathF64<BOX_NONE, false>>(n_stages) : tile_smem_fixed<MathFast<BOX_NONE, 0>>(n_stages);
 }
 
 }  // namespace
@@ -225,9 +225,11 @@ extern "C" int cdh_destroy(cdh_ctx* ctx) {
     if (!ctx) return CDH_OK;
     DeviceGuard g(ctx->device);
     cudaDeviceSynchronize();
+    for (auto& p : ctx->plans) { if (p && p->d_tables) cudaFree(p->d_tables); if (p && p->uploaded) cudaEventDestroy(p->uploaded); }
+    ctx->plans.clear();
     if (ctx->d_pk) cudaFree(ctx->d_pk);
-    if (ctx->d_tables) cudaFree(ctx->d_tables);
     if (ctx->d_scalars) cudaFree(ctx->d_scalars);
+    if (ctx->d_small) cudaFree(ctx->d_small);
     if (ctx->h_tables) cudaFreeHost(ctx->h_tables);
     if (ctx->d_io_coords) cudaFree(ctx->d_io_coords);
     if (ctx->d_io_out) cudaFree(ctx->d_io_out);
@@ -247,151 +249,6 @@ extern "C" int cdh_destroy(cdh_ctx* ctx) {
     return CDH_OK;
 }
 
-// ---- the double-precision call (cdh_f64.cuh): same layout, tables and stream discipline as the fp32 call --------
-typedef void (*TileFn64)(const TileParams64);
-static inline size_t align256(size_t x) { return (x + 255) & ~(size_t)255; }
-
-static int histograms_f64(cdh_ctx* ctx, const double* coords, int32_t n_frames, const int32_t* off, int32_t n_species,
-                          int32_t box_type, const double* box, int32_t n_boxes, double r_max, int32_t n_bins,
-                          cudaStream_t stream, uint64_t* out) {
-    const int nb = (box_type == CDH_BOX_NONE) ? 0 : n_boxes;
-    std::vector<BoxConst64> boxes((size_t)(nb > 0 ? nb : 1));
-    std::memset(boxes.data(), 0, boxes.size() * sizeof(BoxConst64));
-    for (int b = 0; b < nb; ++b) {
-        if (!make_box_const64(box_type, box + 9 * (size_t)b, r_max, &boxes[b])) return CDH_ERR_INVALID_ARG;
-        if (ctx->flags & CDH_FLAG_NO_PRUNE) boxes[b].prune_ok = 0.0;
-    }
-    std::vector<uint32_t> pad_off((size_t)n_species + 1);
-    uint64_t slots = 0;
-    for (int s = 0; s < n_species; ++s) {
-        pad_off[s] = (uint32_t)slots;
-        const uint64_t n = (uint64_t)(off[s + 1] - off[s]);
-        slots += (n + kPadParticles - 1) / kPadParticles * kPadParticles;
-        if (slots > 0x7fffffffull) return CDH_ERR_INVALID_ARG;
-    }
-    pad_off[n_species] = (uint32_t)slots;
-    const uint32_t frame_slots = (uint32_t)slots;
-    if ((uint64_t)frame_slots * (uint64_t)n_frames / kGroup > 0xffffffffull) return CDH_ERR_INVALID_ARG;
-    const int n_hist = n_species * (n_species + 1) / 2;
-
-    DeviceGuard guard(ctx->device);
-    if (!guard.ok) return cuda_fail(ctx, cudaGetLastError(), "cudaSetDevice");
-
-    uint32_t cap_bins = (uint32_t)((ctx->max_smem_optin - tile_smem_bytes64(0)) / 4);
-    const uint32_t flag_cap = ctx->flags >> CDH_FLAG_MAX_SMEM_BINS_SHIFT;
-    if (flag_cap && flag_cap < cap_bins) cap_bins = flag_cap;
-    SweepPlan sp = plan_sweeps((uint32_t)n_bins, cap_bins);
-    const bool global_hist = (ctx->flags & CDH_FLAG_GLOBAL_HIST) != 0 || (!flag_cap && sp.n_sweeps >= kGlobalSweeps);
-    if (global_hist) { sp.n_sweeps = 1; sp.bins_per_sweep = (uint32_t)n_bins; }
-    const int smem_bytes = tile_smem_bytes64(global_hist ? 0 : (int)sp.bins_per_sweep);
-    const bool big = 2 * (smem_bytes + 1024) > 228 * 1024;
-    TileFn64 fn; int threads;
-    const bool pbox = box_type == CDH_BOX_TRICLINIC && nb == 1;      // one box: constants through the parameter bank
-    const bool skip = !big && !global_hist && sp.n_sweeps == 1 && small_species(off, n_species);
-    auto pick64 = [&](auto mode_c) -> TileFn64 {
-        constexpr int M = decltype(mode_c)::value;
-        if constexpr (M == MODE_SHARED)
-            if (skip) {
-                if (box_type == CDH_BOX_NONE) return tile_kernel_f64<BOX_NONE, 256, 2, false, M, true>;
-                if (box_type == CDH_BOX_ORTHO) return tile_kernel_f64<BOX_ORTHO, 256, 2, false, M, true>;
-                return pbox ? tile_kernel_f64<BOX_TRI, 256, 2, true, M, true> : tile_kernel_f64<BOX_TRI, 256, 2, false, M, true>;
-            }
-        if (box_type == CDH_BOX_NONE) return big ? tile_kernel_f64<BOX_NONE, 512, 1, false, M> : tile_kernel_f64<BOX_NONE, 256, 2, false, M>;
-        if (box_type == CDH_BOX_ORTHO) return big ? tile_kernel_f64<BOX_ORTHO, 512, 1, false, M> : tile_kernel_f64<BOX_ORTHO, 256, 2, false, M>;
-        if (pbox) return big ? tile_kernel_f64<BOX_TRI, 512, 1, true, M> : tile_kernel_f64<BOX_TRI, 256, 2, true, M>;
-        return big ? tile_kernel_f64<BOX_TRI, 512, 1, false, M> : tile_kernel_f64<BOX_TRI, 256, 2, false, M>;
-    };
-    fn = global_hist ? pick64(std::integral_constant<int, MODE_GLOBAL>{})
-       : sp.n_sweeps > 1 ? pick64(std::integral_constant<int, MODE_SPLIT>{}) : pick64(std::integral_constant<int, MODE_SHARED>{});
-    threads = big ? 512 : 256;
-    const uint32_t ti = (uint32_t)threads * kR;
-    CDH_CUDA(cudaFuncSetAttribute((const void*)fn, cudaFuncAttributeMaxDynamicSharedMemorySize, smem_bytes));
-    int resident = 0;
-    CDH_CUDA(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&resident, (const void*)fn, threads, (size_t)smem_bytes));
-    if (resident < 1) resident = 1;
-    const uint32_t grid_full = (uint32_t)ctx->n_sm * (uint32_t)resident;
-
-    WorkTables wt;
-    uint32_t tj = 8192;
-    for (;; tj >>= 1) {
-        build_tables(n_frames, off, n_species, nb > 0 ? nb : 1, (uint32_t)n_bins, sp, ti, tj, pad_off, frame_slots, &wt);
-        if (wt.n_items >= kItemsPerCta * grid_full || tj == (uint32_t)kStageParticles) break;
-    }
-    if (wt.n_items >= 0xffffffffull || wt.rows.size() >= 0x7fffffffull) return CDH_ERR_INVALID_ARG;
-
-    const size_t b_segs = align256(wt.segs.size() * sizeof(Seg) + 1), b_rows = align256(wt.rows.size() * sizeof(Row)),
-                 b_boxes = align256(boxes.size() * sizeof(BoxConst64)), b_off = align256(((size_t)n_species + 1) * 4);
-    const size_t tables = b_segs + b_rows + b_boxes + 2 * b_off;
-    int rc;
-    if (ctx->staged_pending) { CDH_CUDA(cudaEventSynchronize(ctx->staged)); ctx->staged_pending = false; }
-    if ((rc = grow(ctx, &ctx->h_tables, &ctx->h_tables_bytes, tables, true)) != CDH_OK) return rc;
-    if ((rc = grow(ctx, &ctx->d_tables, &ctx->tables_bytes, tables, false)) != CDH_OK) return rc;
-    const size_t pk_need = (size_t)n_frames * frame_slots * 3 * sizeof(double);
-    if ((rc = grow(ctx, (void**)&ctx->d_pk, &ctx->pk_bytes, pk_need > 0 ? pk_need : 16, false)) != CDH_OK) return rc;
-
-    char* h = (char*)ctx->h_tables;
-    std::memcpy(h, wt.segs.data(), wt.segs.size() * sizeof(Seg));
-    std::memcpy(h + b_segs, wt.rows.data(), wt.rows.size() * sizeof(Row));
-    std::memcpy(h + b_segs + b_rows, boxes.data(), boxes.size() * sizeof(BoxConst64));
-    std::memcpy(h + b_segs + b_rows + b_boxes, off, ((size_t)n_species + 1) * 4);
-    std::memcpy(h + b_segs + b_rows + b_boxes + b_off, pad_off.data(), ((size_t)n_species + 1) * 4);
-    char* d = (char*)ctx->d_tables;
-    const bool timing = ctx->ev != nullptr;
-    cudaEvent_t* ev = timing ? ctx->ev + 4 * (ctx->timed_calls % CDH_TIMED_CALLS) : nullptr;
-    if (timing) CDH_CUDA(cudaEventRecord(ev[0], stream));
-    CDH_CUDA(cudaMemcpyAsync(d, h, tables, cudaMemcpyHostToDevice, stream));
-    CDH_CUDA(cudaEventRecord(ctx->staged, stream));
-    ctx->staged_pending = true;
-    CDH_CUDA(cudaMemsetAsync(ctx->d_scalars, 0, 64, stream));
-    if (!(ctx->flags & CDH_FLAG_ACCUMULATE))
-        CDH_CUDA(cudaMemsetAsync(out, 0, (size_t)n_hist * (size_t)n_bins * sizeof(uint64_t), stream));
-
-    int launches = 0;
-    if (frame_slots > 0) {
-        RepackParams64 rp;
-        rp.coords = coords; rp.pk = (double*)ctx->d_pk;
-        rp.off = (const int32_t*)(d + b_segs + b_rows + b_boxes);
-        rp.pad_off = (const uint32_t*)(d + b_segs + b_rows + b_boxes + b_off);
-        rp.range_keys = ctx->d_scalars + 4;
-        rp.boxes = (const BoxConst64*)(d + b_segs + b_rows);
-        rp.n_species = n_species; rp.n_total = off[n_species]; rp.n_frames = n_frames;
-        rp.box_type = box_type; rp.n_boxes = nb > 0 ? nb : 1;
-        rp.frame_slots = frame_slots; rp.blocks_per_frame = (frame_slots + 255) / 256;
-        const uint64_t blocks = (uint64_t)rp.blocks_per_frame * (uint64_t)n_frames;
-        if (blocks > 0x7fffffffull) return CDH_ERR_INVALID_ARG;
-        repack_kernel_f64<<<(unsigned)blocks, 256, 0, stream>>>(rp);
-        CDH_CUDA(cudaGetLastError());
-        ++launches;
-    }
-    uint32_t grid = 0;
-    if (timing) CDH_CUDA(cudaEventRecord(ev[1], stream));
-    if (wt.n_items > 0) {
-        TileParams64 tp;
-        tp.pk = (const double*)ctx->d_pk; tp.segs = (const Seg*)d; tp.rows = (const Row*)(d + b_segs);
-        tp.boxes = (const BoxConst64*)(d + b_segs + b_rows);
-        tp.counter = ctx->d_scalars; tp.out = (unsigned long long*)out; tp.range_keys = ctx->d_scalars + 4;
-        tp.n_rows = (uint32_t)wt.rows.size() - 1; tp.n_items = (uint32_t)wt.n_items;
-        tp.n_bins = (uint32_t)n_bins; tp.tj = tj; tp.smem_bins = global_hist ? 0u : sp.bins_per_sweep;
-        tp.rmax = r_max; tp.scale = (double)n_bins / r_max;
-        tp.box0 = boxes[0];
-        grid = grid_full < tp.n_items ? grid_full : tp.n_items;
-        fn<<<grid, threads, smem_bytes, stream>>>(tp);
-        CDH_CUDA(cudaGetLastError());
-        ++launches;
-    }
-    if (timing) {
-        CDH_CUDA(cudaEventRecord(ev[2], stream));
-        CDH_CUDA(cudaEventRecord(ev[3], stream));
-        ++ctx->timed_calls;
-    }
-    ctx->info[0] = launches; ctx->info[1] = (int64_t)wt.n_items; ctx->info[2] = sp.n_sweeps; ctx->info[3] = grid;
-    ctx->info[4] = threads; ctx->info[5] = smem_bytes;
-    ctx->info[6] = 2 | ((int)global_hist << 2) | (box_type << 4) | ((int)(sp.n_sweeps > 1) << 12) | ((int)big << 13) | ((int)skip << 14) |
-                   ((int64_t)tj << 16);
-    ctx->info[7] = (int64_t)wt.padded_pairs;
-    return CDH_OK;
-}
-
 static int validate(const void* coords, int32_t n_frames, const int32_t* off, int32_t n_species, int32_t box_type,
                     const double* box, int32_t n_boxes, double r_max, int32_t n_bins, int32_t precision, const void* out) {
     if (!coords || !off || !out) return CDH_ERR_INVALID_ARG;
@@ -404,34 +261,68 @@ static int validate(const void* coords, int32_t n_frames, const int32_t* off, in
     if (box_type != CDH_BOX_NONE && n_boxes != 1 && n_boxes != n_frames) return CDH_ERR_INVALID_ARG;
     if (off[0] != 0) return CDH_ERR_INVALID_ARG;
     for (int s = 0; s < n_species; ++s) if (off[s + 1] < off[s]) return CDH_ERR_INVALID_ARG;
-    if (!((float)r_max > 0.0f) || !std::isfinite((float)r_max)) return CDH_ERR_INVALID_ARG;
-    const float scale = (float)((double)n_bins / r_max);
-    if (!std::isfinite(scale) || !(scale > 0.0f)) return CDH_ERR_INVALID_ARG;
+    if (precision == CDH_F32) {
+        if (!((float)r_max > 0.0f) || !std::isfinite((float)r_max)) return CDH_ERR_INVALID_ARG;
+        const float scale = (float)((double)n_bins / r_max);
+        if (!std::isfinite(scale) || !(scale > 0.0f)) return CDH_ERR_INVALID_ARG;
+    } else {
+        // the double-precision kernels bin sqrt(d2) < 2^-485 as 0: harmless while it lands in bin 0 and is kept
+        if (!(r_max > 1e-100 && (double)n_bins / r_max < 1e100)) return CDH_ERR_INVALID_ARG;
+    }
     return CDH_OK;
 }
 
-extern "C" int cdh_histograms(cdh_ctx* ctx, const void* coords, int32_t n_frames, const int32_t* off,
-                              int32_t n_species, int32_t box_type, const double* box, int32_t n_boxes,
-                              double r_max, int32_t n_bins, int32_t precision, void* stream_, uint64_t* out) {
-    if (!ctx) return CDH_ERR_INVALID_ARG;
-    int rc = validate(coords, n_frames, off, n_species, box_type, box, n_boxes, r_max, n_bins, precision, out);
-    if (rc != CDH_OK) return rc;
-    cudaStream_t stream = (cudaStream_t)stream_;
-    ctx->err.clear();
-    // the double-precision kernels bin sqrt(d2) < 2^-485 as 0: harmless while it lands in bin 0 and is kept
-    if (precision == CDH_F64 && !(r_max > 1e-100 && (double)n_bins / r_max < 1e100)) return CDH_ERR_INVALID_ARG;
-    if (precision == CDH_F64)
-        return histograms_f64(ctx, (const double*)coords, n_frames, off, n_species, box_type, box, n_boxes, r_max, n_bins, stream, out);
+// ---- plans ---------------------------------------------------------------------------------------------------
+namespace {
+
+std::vector<unsigned char> plan_key(uint32_t flags, int32_t n_frames, const int32_t* off, int32_t n_species, int32_t box_type,
+                                    const double* box, int32_t nb, double r_max, int32_t n_bins, int32_t precision) {
+    const int32_t head[7] = {precision, n_frames, n_species, box_type, nb, n_bins, (int32_t)(flags & ~(uint32_t)CDH_FLAG_ACCUMULATE)};
+    std::vector<unsigned char> k(sizeof head + sizeof r_max + ((size_t)n_species + 1) * 4 + (size_t)nb * 72);
+    unsigned char* w = k.data();
+    std::memcpy(w, head, sizeof head); w += sizeof head;
+    std::memcpy(w, &r_max, sizeof r_max); w += sizeof r_max;
+    std::memcpy(w, off, ((size_t)n_species + 1) * 4); w += ((size_t)n_species + 1) * 4;
+    if (nb > 0) std::memcpy(w, box, (size_t)nb * 72);
+    return k;
+}
+
+#ifndef CDH_GLOBAL_SWEEPS
+#define CDH_GLOBAL_SWEEPS 8   // cross-validation kernels only: shared-memory sweeps from which the global-histogram mode takes
+                              // over (measured break-even: 200,000 uniform points, 400,000 bins: 8 sweeps 200 vs global 221 Gpairs/s)
+#endif
+#ifndef CDH_HYBRID_MAX_RATIO
+#define CDH_HYBRID_MAX_RATIO 16   // production kernels: n_bins / window above which the shared window is dropped (MODE_GLOBAL):
+                                  // it would catch too few pairs to pay for its extra shared update per pair
+#endif
+
+// Builds the plan of a call (host work, table upload on `stream`).  Every argument check happens before the first
+// enqueue; on error nothing was enqueued.
+int build_plan(cdh_ctx* ctx, cudaStream_t stream, int32_t n_frames, const int32_t* off, int32_t n_species, int32_t box_type,
+               const double* box, int32_t n_boxes, double r_max, int32_t n_bins, int32_t precision,
+               std::vector<unsigned char>&& key, Plan** out_plan) {
+    std::unique_ptr<Plan> pl(new (std::nothrow) Plan);
+    if (!pl) return CDH_ERR_ALLOC;
+    const bool f64 = precision == CDH_F64;
+    const int nb = (box_type == CDH_BOX_NONE) ? 0 : n_boxes;
+    const size_t n_box_rec = (size_t)(nb > 0 ? nb : 1);
 
     // ---- host-derived constants ----------------------------------------------------------------
-    const int nb = (box_type == CDH_BOX_NONE) ? 0 : n_boxes;
-    std::vector<BoxConst> boxes((size_t)(nb > 0 ? nb : 1));
-    std::memset(boxes.data(), 0, boxes.size() * sizeof(BoxConst));
+    std::vector<BoxConst> boxes32(f64 ? 0 : n_box_rec);
+    std::vector<BoxConst64> boxes64(f64 ? n_box_rec : 0);
+    if (f64) std::memset(boxes64.data(), 0, boxes64.size() * sizeof(BoxConst64));
+    else std::memset(boxes32.data(), 0, boxes32.size() * sizeof(BoxConst));
+    bool prune_all = true, fused_ok = box_type == CDH_BOX_ORTHO;
     for (int b = 0; b < nb; ++b) {
-        if (!make_box_const(box_type, box + 9 * (size_t)b, r_max, &boxes[b])) return CDH_ERR_INVALID_ARG;
-        if (ctx->flags & CDH_FLAG_NO_PRUNE) boxes[b].prune_ok = 0.0f;
+        if (f64) {
+            if (!make_box_const64(box_type, box + 9 * (size_t)b, r_max, &boxes64[b])) return CDH_ERR_INVALID_ARG;
+            if (ctx->flags & CDH_FLAG_NO_PRUNE) boxes64[b].prune_ok = 0.0;
+        } else {
+            if (!make_box_const(box_type, box + 9 * (size_t)b, r_max, &boxes32[b])) return CDH_ERR_INVALID_ARG;
+            if (boxes32[b].prune_ok == 0.0f) { prune_all = false; fused_ok = false; }
+        }
     }
-    const int tri = (box_type == CDH_BOX_TRICLINIC) ? tri_kind(boxes.data(), nb) : 0;
+    if (ctx->flags & CDH_FLAG_NO_PRUNE) { prune_all = false; fused_ok = false; }   // tests: 27 shifts everywhere / the plain rint form
     const float rmax_f = (float)r_max;
     const float scale_f = (float)((double)n_bins / r_max);
 
@@ -447,59 +338,80 @@ extern "C" int cdh_histograms(cdh_ctx* ctx, const void* coords, int32_t n_frames
     pad_off[n_species] = (uint32_t)slots;
     const uint32_t frame_slots = (uint32_t)slots;
     if ((uint64_t)frame_slots * (uint64_t)n_frames / kGroup > 0xffffffffull) return CDH_ERR_INVALID_ARG;
+    const uint32_t blocks_per_frame = (frame_slots + 255) / 256;
+    if ((uint64_t)blocks_per_frame * (uint64_t)n_frames > 0x7fffffffull) return CDH_ERR_INVALID_ARG;
     const int n_hist = n_species * (n_species + 1) / 2;
+
+    // ---- where the histogram lives -------------------------------------------------------------
+    const bool use_simple_only = !f64 && ((ctx->flags & (CDH_FLAG_SIMPLE_KERNEL | CDH_FLAG_WARP_AGGREGATE | CDH_FLAG_NO_AGGREGATE)) != 0 ||
+                                          !(scale_f < 5.0e14f));
+    const uint32_t cap_ring = (uint32_t)((ctx->max_smem_optin - smem_fixed(precision, CDH_STAGES)) / 4 - 2);   // bins next to the full ring
+    const uint32_t cap_two = (uint32_t)((ctx->max_smem_optin - smem_fixed(precision, 2)) / 4 - 2);              // ... next to two stages
+    const uint32_t flag_cap = ctx->flags >> CDH_FLAG_MAX_SMEM_BINS_SHIFT;
+    SweepPlan sp; sp.n_sweeps = 1; sp.bins_per_sweep = (uint32_t)n_bins;
+    int mode = MODE_SHARED;
+    uint32_t smem_bins = (uint32_t)n_bins, n_stages = CDH_STAGES;
+    if (ctx->flags & CDH_FLAG_GLOBAL_HIST) { mode = MODE_GLOBAL; smem_bins = 0; }
+    else if (flag_cap && flag_cap < (uint32_t)n_bins) {                      // tests: force the bin-range split
+        sp = plan_sweeps((uint32_t)n_bins, std::min(flag_cap, cap_two));
+        mode = MODE_SPLIT; smem_bins = sp.bins_per_sweep;
+    } else if ((uint32_t)n_bins > cap_two) {                                 // wider than a CTA's shared memory
+        if (use_simple_only) {
+            sp = plan_sweeps((uint32_t)n_bins, cap_two);
+            if (sp.n_sweeps >= CDH_GLOBAL_SWEEPS) { sp.n_sweeps = 1; sp.bins_per_sweep = (uint32_t)n_bins; mode = MODE_GLOBAL; smem_bins = 0; }
+            else { mode = MODE_SPLIT; smem_bins = sp.bins_per_sweep; }
+        } else if ((uint64_t)n_bins > (uint64_t)CDH_HYBRID_MAX_RATIO * cap_two) { mode = MODE_GLOBAL; smem_bins = 0; }
+        else { mode = MODE_HYBRID; smem_bins = cap_two; }
+    }
+    if (mode != MODE_GLOBAL && smem_bins > cap_ring) n_stages = 2;
+    const int smem_bytes = smem_fixed(precision, (int)n_stages) + 4 * ((int)smem_bins + 2);
+    const bool big = 2 * (smem_bytes + 1024) > 228 * 1024 || mode == MODE_HYBRID;          // one CTA per SM
+    const bool skip = !big && mode == MODE_SHARED && !use_simple_only && small_species(off, n_species);
+    const int shape = big ? SHAPE_BIG : (skip ? SHAPE_256_SKIP : SHAPE_256);
+
+    // ---- launch plan ----------------------------------------------------------------------------
+    // Every tile launch of the call owns an interval (lo, hi] of the fractional-coordinate range the repack kernel
+    // measures, and exactly one of them does the work (cdh_math32.cuh launch_begin).
+    //   ORTHO: fused rint up to 1.49 (exact-product form if the host found no fused constants for some box),
+    //          magic-number rint up to 2^20, library rintf beyond;  TRICLINIC: fast path up to 1.49 (n in {-1,0,1}),
+    //          wide fast path up to 64, definition beyond.
+    const float kInf = INFINITY, kSmall = 1.49f, kWide = 64.0f, kMagic = 1048576.0f;
+    int form = 0;
+    bool pbox = false;
+    if (f64) {
+        pbox = box_type == CDH_BOX_TRICLINIC && nb == 1;      // one box: constants through the parameter bank
+        pl->launches.push_back({f64_variant(box_type, pbox, mode, shape), -kInf, kInf});
+    } else {
+        const int simple_mode = (mode == MODE_SHARED || mode == MODE_SPLIT) ? MODE_SPLIT : MODE_GLOBAL;
+        const int var = (ctx->flags & CDH_FLAG_WARP_AGGREGATE) ? VAR_SIMPLE_MATCH : (ctx->flags & CDH_FLAG_NO_AGGREGATE) ? VAR_SIMPLE_PLAIN : VAR_SIMPLE;
+        const Variant vs = simple_variant(box_type, var, simple_mode, big ? SHAPE_BIG : SHAPE_256);
+        auto fast_of = [&](int f) { return fast_variant(box_type, f, mode, shape); };
+        if (use_simple_only) pl->launches.push_back({vs, -kInf, kInf});
+        else if (box_type == CDH_BOX_NONE) pl->launches.push_back({fast_of(0), -kInf, kInf});
+        else if (box_type == CDH_BOX_ORTHO) {
+            const bool plain_only = (ctx->flags & CDH_FLAG_NO_PRUNE) != 0;     // tests: the pinned 5-operation form everywhere
+            form = plain_only ? ORTHO_PLAIN : fused_ok ? ORTHO_FUSED : ORTHO_EXACT;
+            if (plain_only) pl->launches.push_back({fast_of(ORTHO_PLAIN), -kInf, kMagic});
+            else { pl->launches.push_back({fast_of(form), -kInf, kSmall}); pl->launches.push_back({fast_of(ORTHO_PLAIN), kSmall, kMagic}); }
+            pl->launches.push_back({vs, kMagic, kInf});
+        } else {
+            // all boxes prunable: the zero structure shared by B and B^-1 picks the form; else the 27-shift search for every pair
+            form = prune_all ? tri_kind(boxes32.data(), nb) : (TRI_GENERAL | TRI_NOPRUNE);
+            pl->launches.push_back({fast_of(form), -kInf, kSmall});
+            pl->launches.push_back({fast_of(form | TRI_WIDE), kSmall, kWide});      // unwrapped coordinates, up to 64 cells
+            pl->launches.push_back({vs, kWide, kInf});
+        }
+    }
+    for (const Launch& l : pl->launches) if (!l.v.fn) { ctx->err = "kernel variant not built"; return CDH_ERR_UNSUPPORTED; }
+    const Variant vf = pl->launches[0].v;
+    const uint32_t ti = (uint32_t)vf.threads * kR;
 
     DeviceGuard guard(ctx->device);
     if (!guard.ok) return cuda_fail(ctx, cudaGetLastError(), "cudaSetDevice");
-
-    // ---- variant, sweeps, tile sizes -----------------------------------------------------------
-    uint32_t cap_bins = (uint32_t)((ctx->max_smem_optin - tile_smem_bytes(0)) / 4);
-    const uint32_t flag_cap = ctx->flags >> CDH_FLAG_MAX_SMEM_BINS_SHIFT;
-    if (flag_cap && flag_cap < cap_bins) cap_bins = flag_cap;
-    SweepPlan sp = plan_sweeps((uint32_t)n_bins, cap_bins);
-    // Very wide histograms (the paper's global-memory kernel regime): beyond kGlobalSweeps
-    // sweeps the private copy is dropped and updates go straight to the uint64 result in L2 (MODE_GLOBAL).
-    const bool global_hist = (ctx->flags & CDH_FLAG_GLOBAL_HIST) != 0 || (!flag_cap && sp.n_sweeps >= kGlobalSweeps);
-    if (global_hist) { sp.n_sweeps = 1; sp.bins_per_sweep = (uint32_t)n_bins; }
-    const int smem_bytes = tile_smem_bytes(global_hist ? 0 : (int)sp.bins_per_sweep);
-    const bool big = 2 * (smem_bytes + 1024) > 228 * 1024;          // one CTA per SM
-    const bool split = sp.n_sweeps > 1;
-    const bool use_simple_only = (ctx->flags & (CDH_FLAG_SIMPLE_KERNEL | CDH_FLAG_WARP_AGGREGATE | CDH_FLAG_NO_AGGREGATE)) != 0 ||
-                                 !(scale_f < 5.0e14f);
-    // Launch plan: every tile launch of the call owns an interval (lo, hi] of the fractional-coordinate range the
-    // repack kernel measures, and exactly one of them does the work (cdh_tile.cuh).
-    //   ORTHO: fused rint up to 1.49 (exact-product form if the host found no fused constants for some box),
-    //          magic-number rint up to 2^20, library rintf beyond;  TRICLINIC: fast path up to 1.49 (n in {-1,0,1}), wide fast path up to 64,
-    //          definition beyond.
-    struct Launch { Variant v; float lo, hi; };
-    const float kInf = INFINITY, kSmall = 1.49f, kWide = 64.0f, kMagic = 1048576.0f;
-    bool fused_ok = box_type == CDH_BOX_ORTHO;
-    for (int b = 0; b < nb && fused_ok; ++b) fused_ok = boxes[b].prune_ok != 0.0f;
-    if (ctx->flags & CDH_FLAG_NO_PRUNE) fused_ok = false;          // tests: force the plain magic-number form
-    const bool skip = small_species(off, n_species);
-    auto fast_of = [&](int form) {
-        return global_hist ? pick_fast<MODE_GLOBAL>(box_type, form, big, false)
-                           : split ? pick_fast<MODE_SPLIT>(box_type, form, big, false) : pick_fast<MODE_SHARED>(box_type, form, big, skip);
-    };
-    const Variant vs = global_hist ? simple_global(box_type) : pick_simple(box_type, big, ctx->flags);
-    std::vector<Launch> plan;
-    if (use_simple_only) plan.push_back({vs, -kInf, kInf});
-    else if (box_type == CDH_BOX_NONE) plan.push_back({fast_of(0), -kInf, kInf});
-    else if (box_type == CDH_BOX_ORTHO) {
-        const bool plain_only = (ctx->flags & CDH_FLAG_NO_PRUNE) != 0;     // tests: the pinned 5-operation form everywhere
-        if (plain_only) plan.push_back({fast_of(ORTHO_PLAIN), -kInf, kMagic});
-        else { plan.push_back({fast_of(fused_ok ? ORTHO_FUSED : ORTHO_EXACT), -kInf, kSmall}); plan.push_back({fast_of(ORTHO_PLAIN), kSmall, kMagic}); }
-        plan.push_back({vs, kMagic, kInf});
-    } else {
-        plan.push_back({fast_of(tri), -kInf, kSmall});
-        plan.push_back({fast_of(tri | TRI_WIDE), kSmall, kWide});      // unwrapped coordinates, up to 64 cells
-        plan.push_back({vs, kWide, kInf});
-    }
-    const Variant vf = plan[0].v;
-    const uint32_t ti = (uint32_t)vf.threads * kR;
-    CDH_CUDA(cudaFuncSetAttribute((const void*)vf.fn, cudaFuncAttributeMaxDynamicSharedMemorySize, smem_bytes));
+    for (const Launch& l : pl->launches)
+        CDH_CUDA(cudaFuncSetAttribute(l.v.fn, cudaFuncAttributeMaxDynamicSharedMemorySize, smem_bytes));
     int resident = 0;      // CTAs of the production variant that fit one SM (registers, shared memory)
-    CDH_CUDA(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&resident, (const void*)vf.fn, vf.threads, (size_t)smem_bytes));
+    CDH_CUDA(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&resident, vf.fn, vf.threads, (size_t)smem_bytes));
     if (resident < 1) resident = 1;
     const uint32_t grid_full = (uint32_t)ctx->n_sm * (uint32_t)resident;
 
@@ -510,72 +422,151 @@ extern "C" int cdh_histograms(cdh_ctx* ctx, const void* coords, int32_t n_frames
         if (wt.n_items >= kItemsPerCta * grid_full || tj == (uint32_t)kStageParticles) break;
     }
     if (wt.n_items >= 0xffffffffull || wt.rows.size() >= 0x7fffffffull) return CDH_ERR_INVALID_ARG;
+    std::vector<int32_t> row_seg((size_t)n_hist, -1);          // first segment of each histogram row (window_kernel)
+    for (size_t k = wt.segs.size(); k-- > 0;) row_seg[wt.segs[k].hist] = (int32_t)k;
 
-    // ---- scratch -------------------------------------------------------------------------------
+    // ---- tables: staged in pinned memory, uploaded once into the plan's own device buffer --------------------------
+    const size_t box_rec = f64 ? sizeof(BoxConst64) : sizeof(BoxConst);
     const size_t b_segs = align256(wt.segs.size() * sizeof(Seg) + 1), b_rows = align256(wt.rows.size() * sizeof(Row)),
-                 b_boxes = align256(boxes.size() * sizeof(BoxConst)), b_off = align256(((size_t)n_species + 1) * 4);
-    const size_t tables = b_segs + b_rows + b_boxes + 2 * b_off;
+                 b_boxes = align256(n_box_rec * box_rec), b_off = align256(((size_t)n_species + 1) * 4),
+                 b_rowseg = align256((size_t)n_hist * 4);
+    pl->o_rows = b_segs; pl->o_boxes = pl->o_rows + b_rows; pl->o_off = pl->o_boxes + b_boxes; pl->o_pad = pl->o_off + b_off;
+    pl->o_rowseg = pl->o_pad + b_off; pl->o_win = pl->o_rowseg + b_rowseg;
+    const size_t tables = pl->o_win + b_rowseg;
+    int rc;
     if (ctx->staged_pending) { CDH_CUDA(cudaEventSynchronize(ctx->staged)); ctx->staged_pending = false; }
     if ((rc = grow(ctx, &ctx->h_tables, &ctx->h_tables_bytes, tables, true)) != CDH_OK) return rc;
-    if ((rc = grow(ctx, &ctx->d_tables, &ctx->tables_bytes, tables, false)) != CDH_OK) return rc;
-    const size_t pk_need = (size_t)n_frames * frame_slots * 3 * sizeof(float);
-    if ((rc = grow(ctx, (void**)&ctx->d_pk, &ctx->pk_bytes, pk_need > 0 ? pk_need : 16, false)) != CDH_OK) return rc;
-
+    const size_t pk_need = (size_t)n_frames * frame_slots * 3 * (f64 ? sizeof(double) : sizeof(float));
+    if ((rc = grow(ctx, &ctx->d_pk, &ctx->pk_bytes, pk_need > 0 ? pk_need : 16, false)) != CDH_OK) return rc;
+    if (cudaMalloc(&pl->d_tables, tables) != cudaSuccess) { cudaGetLastError(); pl->d_tables = nullptr; ctx->err = "plan tables"; return CDH_ERR_ALLOC; }
     char* h = (char*)ctx->h_tables;
+    std::memset(h, 0, tables);
     std::memcpy(h, wt.segs.data(), wt.segs.size() * sizeof(Seg));
-    std::memcpy(h + b_segs, wt.rows.data(), wt.rows.size() * sizeof(Row));
-    std::memcpy(h + b_segs + b_rows, boxes.data(), boxes.size() * sizeof(BoxConst));
-    std::memcpy(h + b_segs + b_rows + b_boxes, off, ((size_t)n_species + 1) * 4);
-    std::memcpy(h + b_segs + b_rows + b_boxes + b_off, pad_off.data(), ((size_t)n_species + 1) * 4);
-    char* d = (char*)ctx->d_tables;
+    std::memcpy(h + pl->o_rows, wt.rows.data(), wt.rows.size() * sizeof(Row));
+    std::memcpy(h + pl->o_boxes, f64 ? (const void*)boxes64.data() : (const void*)boxes32.data(), n_box_rec * box_rec);
+    std::memcpy(h + pl->o_off, off, ((size_t)n_species + 1) * 4);
+    std::memcpy(h + pl->o_pad, pad_off.data(), ((size_t)n_species + 1) * 4);
+    std::memcpy(h + pl->o_rowseg, row_seg.data(), (size_t)n_hist * 4);
+    cudaError_t e = cudaEventCreateWithFlags(&pl->uploaded, cudaEventDisableTiming);
+    if (e == cudaSuccess) e = cudaMemcpyAsync(pl->d_tables, h, tables, cudaMemcpyHostToDevice, stream);
+    if (e == cudaSuccess) e = cudaEventRecord(ctx->staged, stream);
+    if (e == cudaSuccess) e = cudaEventRecord(pl->uploaded, stream);
+    if (e != cudaSuccess) {
+        cudaFree(pl->d_tables); pl->d_tables = nullptr;
+        if (pl->uploaded) cudaEventDestroy(pl->uploaded);
+        return cuda_fail(ctx, e, "plan table upload");
+    }
+    ctx->staged_pending = true;
+    pl->up_stream = stream;
+
+    pl->key = std::move(key);
+    pl->pk_bytes = pk_need;
+    pl->precision = precision; pl->box_type = box_type; pl->n_hist = n_hist; pl->n_species = n_species; pl->n_frames = n_frames;
+    pl->n_boxes = nb > 0 ? nb : 1; pl->n_total = off[n_species];
+    pl->n_bins = (uint32_t)n_bins; pl->frame_slots = frame_slots; pl->blocks_per_frame = blocks_per_frame;
+    pl->repack_blocks = blocks_per_frame * (uint32_t)n_frames;
+    pl->smem_bytes = smem_bytes; pl->mode = mode; pl->n_items = (uint32_t)wt.n_items; pl->n_rows = (uint32_t)wt.rows.size() - 1;
+    pl->grid = grid_full < pl->n_items ? grid_full : pl->n_items;
+    pl->tj = tj; pl->smem_bins = smem_bins; pl->n_stages = n_stages;
+    pl->r_max = r_max; pl->rmax_f = rmax_f; pl->scale_f = scale_f; pl->thr2_bits = f64 ? 0u : d2_threshold_bits(rmax_f);
+    if (f64) pl->box0_64 = boxes64[0];
+    const int n_launch = (frame_slots > 0 ? 1 : 0) + (wt.n_items > 0 ? (int)pl->launches.size() + (mode == MODE_HYBRID ? 1 : 0) : 0);
+    pl->info[0] = n_launch; pl->info[1] = (int64_t)wt.n_items; pl->info[2] = sp.n_sweeps; pl->info[3] = pl->grid;
+    pl->info[4] = vf.threads; pl->info[5] = smem_bytes;
+    pl->info[6] = (f64 ? 2 : (use_simple_only ? 0 : 1)) | ((int)(mode == MODE_GLOBAL) << 2) | ((int)(mode == MODE_HYBRID) << 3) | (box_type << 4) |
+                  ((form & 15) << 8) | ((int)(mode == MODE_SPLIT) << 12) | ((int)big << 13) | ((int)skip << 14) | ((int64_t)tj << 16);
+    pl->info[7] = (int64_t)wt.padded_pairs;
+
+    // least recently used plan out (its tables may still be read by enqueued work: wait for the device first)
+    if (ctx->plans.size() >= kMaxPlans) {
+        size_t victim = 0;
+        for (size_t k = 1; k < ctx->plans.size(); ++k) if (ctx->plans[k]->stamp < ctx->plans[victim]->stamp) victim = k;
+        cudaDeviceSynchronize();
+        if (ctx->plans[victim]->d_tables) cudaFree(ctx->plans[victim]->d_tables);
+        if (ctx->plans[victim]->uploaded) cudaEventDestroy(ctx->plans[victim]->uploaded);
+        ctx->plans.erase(ctx->plans.begin() + (long)victim);
+    }
+    *out_plan = pl.get();
+    ctx->plans.push_back(std::move(pl));
+    return CDH_OK;
+}
+
+// Enqueues the call on `stream`: zeroing, repack, (window), tile launch(es).
+int enqueue_plan(cdh_ctx* ctx, const Plan& pl, const void* coords, cudaStream_t stream, uint64_t* out) {
+    DeviceGuard guard(ctx->device);
+    if (!guard.ok) return cuda_fail(ctx, cudaGetLastError(), "cudaSetDevice");
+    const bool f64 = pl.precision == CDH_F64;
+    char* d = (char*)pl.d_tables;
     const bool timing = ctx->ev != nullptr;
     cudaEvent_t* ev = timing ? ctx->ev + 4 * (ctx->timed_calls % CDH_TIMED_CALLS) : nullptr;
+    if (stream != pl.up_stream) CDH_CUDA(cudaStreamWaitEvent(stream, pl.uploaded, 0));   // the tables went up on another stream
     if (timing) CDH_CUDA(cudaEventRecord(ev[0], stream));
-    CDH_CUDA(cudaMemcpyAsync(d, h, tables, cudaMemcpyHostToDevice, stream));
-    CDH_CUDA(cudaEventRecord(ctx->staged, stream));
-    ctx->staged_pending = true;
     CDH_CUDA(cudaMemsetAsync(ctx->d_scalars, 0, 64, stream));
     if (!(ctx->flags & CDH_FLAG_ACCUMULATE))
-        CDH_CUDA(cudaMemsetAsync(out, 0, (size_t)n_hist * (size_t)n_bins * sizeof(uint64_t), stream));
+        CDH_CUDA(cudaMemsetAsync(out, 0, (size_t)pl.n_hist * (size_t)pl.n_bins * sizeof(uint64_t), stream));
 
-    int launches = 0;
     // ---- K0 repack -----------------------------------------------------------------------------
-    if (frame_slots > 0) {
-        RepackParams rp;
-        rp.coords = (const float*)coords; rp.pk = ctx->d_pk;
-        rp.off = (const int32_t*)(d + b_segs + b_rows + b_boxes);
-        rp.pad_off = (const uint32_t*)(d + b_segs + b_rows + b_boxes + b_off);
-        rp.range_keys = ctx->d_scalars + 4;
-        rp.boxes = (const BoxConst*)(d + b_segs + b_rows);
-        rp.n_species = n_species; rp.n_total = off[n_species]; rp.n_frames = n_frames;
-        rp.box_type = box_type; rp.n_boxes = nb > 0 ? nb : 1;
-        rp.frame_slots = frame_slots; rp.blocks_per_frame = (frame_slots + 255) / 256;
-        const uint64_t blocks = (uint64_t)rp.blocks_per_frame * (uint64_t)n_frames;
-        if (blocks > 0x7fffffffull) return CDH_ERR_INVALID_ARG;
-        repack_kernel<<<(unsigned)blocks, 256, 0, stream>>>(rp);
+    if (pl.frame_slots > 0) {
+        if (f64) {
+            RepackParams64 rp;
+            rp.coords = (const double*)coords; rp.pk = (double*)ctx->d_pk;
+            rp.off = (const int32_t*)(d + pl.o_off); rp.pad_off = (const uint32_t*)(d + pl.o_pad);
+            rp.range_keys = ctx->d_scalars + 4; rp.boxes = (const BoxConst64*)(d + pl.o_boxes);
+            rp.n_species = pl.n_species; rp.n_total = pl.n_total; rp.n_frames = pl.n_frames;
+            rp.box_type = pl.box_type; rp.n_boxes = pl.n_boxes;
+            rp.frame_slots = pl.frame_slots; rp.blocks_per_frame = pl.blocks_per_frame;
+            repack_kernel_f64<<<pl.repack_blocks, 256, 0, stream>>>(rp);
+        } else {
+            RepackParams rp;
+            rp.coords = (const float*)coords; rp.pk = (float*)ctx->d_pk;
+            rp.off = (const int32_t*)(d + pl.o_off); rp.pad_off = (const uint32_t*)(d + pl.o_pad);
+            rp.range_keys = ctx->d_scalars + 4; rp.boxes = (const BoxConst*)(d + pl.o_boxes);
+            rp.n_species = pl.n_species; rp.n_total = pl.n_total; rp.n_frames = pl.n_frames;
+            rp.box_type = pl.box_type; rp.n_boxes = pl.n_boxes;
+            rp.frame_slots = pl.frame_slots; rp.blocks_per_frame = pl.blocks_per_frame;
+            repack_kernel<<<pl.repack_blocks, 256, 0, stream>>>(rp);
+        }
         CDH_CUDA(cudaGetLastError());
-        ++launches;
     }
 
     // ---- K1 tile kernel(s) ---------------------------------------------------------------------
-    uint32_t grid = 0;
     if (timing) CDH_CUDA(cudaEventRecord(ev[1], stream));
-    if (wt.n_items > 0) {
-        TileParams tp;
-        tp.pk = ctx->d_pk; tp.segs = (const Seg*)d; tp.rows = (const Row*)(d + b_segs);
-        tp.boxes = (const BoxConst*)(d + b_segs + b_rows);
-        tp.out = (unsigned long long*)out; tp.range_keys = ctx->d_scalars + 4;
-        tp.n_rows = (uint32_t)wt.rows.size() - 1; tp.n_items = (uint32_t)wt.n_items;
-        tp.n_bins = (uint32_t)n_bins; tp.tj = tj; tp.smem_bins = global_hist ? 0u : sp.bins_per_sweep;
-        tp.rmax = rmax_f; tp.scale = scale_f; tp.thr2_bits = d2_threshold_bits(rmax_f); tp.one = 1.0f;
-        grid = grid_full < tp.n_items ? grid_full : tp.n_items;
-        for (size_t k = 0; k < plan.size(); ++k) {
-            tp.counter = ctx->d_scalars + k;
-            tp.range_lo = plan[k].lo; tp.range_hi = plan[k].hi;
-            if (k > 0) CDH_CUDA(cudaFuncSetAttribute((const void*)plan[k].v.fn, cudaFuncAttributeMaxDynamicSharedMemorySize, smem_bytes));
-            plan[k].v.fn<<<grid, plan[k].v.threads, smem_bytes, stream>>>(tp);
+    if (pl.n_items > 0) {
+        TileParams tp; TileParams64 tp64;
+        TileCommon& c = f64 ? static_cast<TileCommon&>(tp64) : static_cast<TileCommon&>(tp);
+        c.segs = (const Seg*)d; c.rows = (const Row*)(d + pl.o_rows);
+        c.out = (unsigned long long*)out; c.range_keys = ctx->d_scalars + 4; c.win_lo = (const uint32_t*)(d + pl.o_win);
+        c.n_rows = pl.n_rows; c.n_items = pl.n_items; c.n_bins = pl.n_bins; c.tj = pl.tj; c.smem_bins = pl.smem_bins;
+        c.n_stages = pl.n_stages;
+        if (f64) {
+            tp64.pk = (const double*)ctx->d_pk; tp64.boxes = (const BoxConst64*)(d + pl.o_boxes);
+            tp64.rmax = pl.r_max; tp64.scale = (double)pl.n_bins / pl.r_max; tp64.box0 = pl.box0_64;
+        } else {
+            tp.pk = (const float*)ctx->d_pk; tp.boxes = (const BoxConst*)(d + pl.o_boxes);
+            tp.rmax = pl.rmax_f; tp.scale = pl.scale_f; tp.thr2_bits = pl.thr2_bits; tp.one = 1.0f; tp.one_u = 1.0f;
+        }
+        if (pl.mode == MODE_HYBRID) {       // K0b: the shared-memory window of every histogram row
+            if (f64) {
+                WindowParams<double, BoxConst64> wp;
+                wp.pk = tp64.pk; wp.segs = c.segs; wp.row_seg = (const int32_t*)(d + pl.o_rowseg); wp.boxes = tp64.boxes;
+                wp.win_lo = (uint32_t*)(d + pl.o_win); wp.box_type = pl.box_type; wp.n_bins = pl.n_bins; wp.window = pl.smem_bins;
+                wp.scale = (float)((double)pl.n_bins / pl.r_max);
+                window_kernel<double, BoxConst64><<<pl.n_hist, 256, 0, stream>>>(wp);
+            } else {
+                WindowParams<float, BoxConst> wp;
+                wp.pk = tp.pk; wp.segs = c.segs; wp.row_seg = (const int32_t*)(d + pl.o_rowseg); wp.boxes = tp.boxes;
+                wp.win_lo = (uint32_t*)(d + pl.o_win); wp.box_type = pl.box_type; wp.n_bins = pl.n_bins; wp.window = pl.smem_bins;
+                wp.scale = pl.scale_f;
+                window_kernel<float, BoxConst><<<pl.n_hist, 256, 0, stream>>>(wp);
+            }
             CDH_CUDA(cudaGetLastError());
-            ++launches;
+        }
+        for (size_t k = 0; k < pl.launches.size(); ++k) {
+            c.counter = ctx->d_scalars + k;
+            if (!f64) { tp.range_lo = pl.launches[k].lo; tp.range_hi = pl.launches[k].hi; }
+            void* args[1] = {f64 ? (void*)&tp64 : (void*)&tp};
+            CDH_CUDA(cudaLaunchKernel(pl.launches[k].v.fn, dim3(pl.grid), dim3((unsigned)pl.launches[k].v.threads), args,
+                                      (size_t)pl.smem_bytes, stream));
         }
     }
     if (timing) {
@@ -583,14 +574,31 @@ extern "C" int cdh_histograms(cdh_ctx* ctx, const void* coords, int32_t n_frames
         CDH_CUDA(cudaEventRecord(ev[3], stream));
         ++ctx->timed_calls;
     }
-    ctx->info[0] = launches; ctx->info[1] = (int64_t)wt.n_items; ctx->info[2] = sp.n_sweeps; ctx->info[3] = grid;
-    ctx->info[4] = vf.threads; ctx->info[5] = smem_bytes;
-    const int form = box_type == CDH_BOX_ORTHO ? ((ctx->flags & CDH_FLAG_NO_PRUNE) ? ORTHO_PLAIN : fused_ok ? ORTHO_FUSED : ORTHO_EXACT) : tri;
-    const bool skip_used = skip && !big && !split && !global_hist && !use_simple_only;
-    ctx->info[6] = (use_simple_only ? 0 : 1) | ((int)global_hist << 2) | (box_type << 4) | (form << 8) | ((int)split << 12) | ((int)big << 13) |
-                   ((int)skip_used << 14) | ((int64_t)tj << 16);
-    ctx->info[7] = (int64_t)wt.padded_pairs;
+    for (int k = 0; k < 8; ++k) ctx->info[k] = pl.info[k];
     return CDH_OK;
+}
+
+}  // namespace
+
+extern "C" int cdh_histograms(cdh_ctx* ctx, const void* coords, int32_t n_frames, const int32_t* off,
+                              int32_t n_species, int32_t box_type, const double* box, int32_t n_boxes,
+                              double r_max, int32_t n_bins, int32_t precision, void* stream_, uint64_t* out) {
+    if (!ctx) return CDH_ERR_INVALID_ARG;
+    int rc = validate(coords, n_frames, off, n_species, box_type, box, n_boxes, r_max, n_bins, precision, out);
+    if (rc != CDH_OK) return rc;
+    cudaStream_t stream = (cudaStream_t)stream_;
+    ctx->err.clear();
+    const int nb = (box_type == CDH_BOX_NONE) ? 0 : n_boxes;
+    std::vector<unsigned char> key = plan_key(ctx->flags, n_frames, off, n_species, box_type, box, nb, r_max, n_bins, precision);
+    Plan* pl = nullptr;
+    for (auto& p : ctx->plans)
+        if (p->key.size() == key.size() && std::memcmp(p->key.data(), key.data(), key.size()) == 0) { pl = p.get(); break; }
+    if (!pl) {
+        rc = build_plan(ctx, stream, n_frames, off, n_species, box_type, box, n_boxes, r_max, n_bins, precision, std::move(key), &pl);
+        if (rc != CDH_OK) return rc;
+    }
+    pl->stamp = ++ctx->stamp;
+    return enqueue_plan(ctx, *pl, coords, stream, out);
 }
 
 extern "C" int cdh_histograms_host(cdh_ctx* ctx, const void* coords, int32_t n_frames, const int32_t* off,
@@ -705,14 +713,14 @@ extern "C" int cdh_rdf(cdh_ctx* ctx, const uint64_t* hist, int32_t n_hist, int32
     const size_t bytes = (size_t)n_hist * sizeof(double);
     if (ctx->staged_pending) { CDH_CUDA(cudaEventSynchronize(ctx->staged)); ctx->staged_pending = false; }
     if ((rc = grow(ctx, &ctx->h_tables, &ctx->h_tables_bytes, bytes, true)) != CDH_OK) return rc;
-    if ((rc = grow(ctx, &ctx->d_tables, &ctx->tables_bytes, bytes, false)) != CDH_OK) return rc;
+    if ((rc = grow(ctx, &ctx->d_small, &ctx->small_bytes, bytes, false)) != CDH_OK) return rc;
     double* hd = (double*)ctx->h_tables;
     for (int h = 0; h < n_hist; ++h) hd[h] = n_pairs[h] / volume;
-    CDH_CUDA(cudaMemcpyAsync(ctx->d_tables, hd, bytes, cudaMemcpyHostToDevice, stream));
+    CDH_CUDA(cudaMemcpyAsync(ctx->d_small, hd, bytes, cudaMemcpyHostToDevice, stream));
     CDH_CUDA(cudaEventRecord(ctx->staged, stream));
     ctx->staged_pending = true;
     RdfParams rp;
-    rp.hist = (const unsigned long long*)hist; rp.density = (const double*)ctx->d_tables; rp.g = g;
+    rp.hist = (const unsigned long long*)hist; rp.density = (const double*)ctx->d_small; rp.g = g;
     rp.dr = r_max / (double)n_bins; rp.n_frames = (double)n_frames; rp.n_bins = (uint32_t)n_bins;
     rp.total = (uint64_t)n_hist * (uint64_t)n_bins;
     const uint64_t blocks = (rp.total + 255) / 256;

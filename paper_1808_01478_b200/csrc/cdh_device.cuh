@@ -63,21 +63,31 @@ struct BoxConst {
 };
 static_assert(sizeof(BoxConst) % 16 == 0, "BoxConst is copied and indexed in 16-byte units");
 
-struct TileParams {
-    const float*    pk;         // repacked coordinates
+// The part of the tile kernel's parameters that does not depend on the precision (cdh_sched.cuh).
+struct TileCommon {
     const Seg*      segs;
     const Row*      rows;       // n_rows + 1 entries (last: item_prefix = n_items)
-    const BoxConst* boxes;
     unsigned int*   counter;    // dynamic work counter (zeroed before the launch)
     unsigned long long* out;    // uint64 [n_hist][n_bins]
-    const unsigned int* range_keys;  // device, written by the repack kernel: min / max keys of the fractional coordinates
+    const unsigned int* range_keys;  // device, written by the repack kernel: [0..2] max keys, [3..5] complemented min keys of the
+                                     // fractional coordinates (periodic boxes) or of the raw coordinates (no box), [6] != 0: some
+                                     // particle has a NaN coordinate
+    const uint32_t* win_lo;     // MODE_HYBRID: first bin of the shared-memory window of each histogram row (device; window_kernel)
     uint32_t n_rows, n_items;
     uint32_t n_bins;
     uint32_t tj;                // j-chunk size in particles (multiple of kStageParticles)
-    uint32_t smem_bins;         // capacity of the shared histogram (bins per sweep, without the extra slot)
+    uint32_t smem_bins;         // capacity of the shared histogram (bins per sweep / window, without the two extra slots)
+    uint32_t n_stages;          // stages of the TMA ring (power of two, 2..8)
+};
+
+struct TileParams : TileCommon {
+    const float*    pk;         // repacked coordinates
+    const BoxConst* boxes;
     float rmax, scale;          // (float)r_max, (float)(n_bins / r_max)
     uint32_t thr2_bits;         // bits of the smallest fp32 d2 whose correctly rounded sqrt is >= rmax
     float one;                  // 1.0f, opaque to ptxas: keeps packed mul/add pairs unfused
+    float one_u;                // 1.0f once more, for FFMA2 whose other two operands are register pairs: ptxas keeps this copy
+                                // in a uniform register (the first one must be a vector register where the addend is an immediate)
     float range_lo, range_hi;   // periodic boxes: this launch does the work iff range_lo < frac_range() <= range_hi
                                 // (range_hi = +inf: no upper limit, and a NaN range counts as above range_lo)
 };

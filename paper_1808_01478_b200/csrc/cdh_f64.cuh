@@ -7,9 +7,9 @@
 // DESIGN.md "Triclinic pruning"; the margins are far wider in double).
 //
 // Layout: groups of 4 particles, 12 doubles per group  x0..3 | y0..3 | z0..3  (96 bytes), NaN padded like the fp32
-// buffer; a j-stage is 256 particles = 6 KB, two stages filled by 1-D TMA bulk copies.
+// buffer; a j-stage is 256 particles = 6 KB, the ring of stages is filled by 1-D TMA bulk copies (cdh_sched.cuh).
 #pragma once
-#include "cdh_tile.cuh"
+#include "cdh_kernels.cuh"
 #include "cdh_sqrt64.cuh"
 
 namespace cdh {
@@ -24,26 +24,13 @@ struct BoxConst64 {
     double pad_;
 };
 
-struct TileParams64 {
+struct TileParams64 : TileCommon {
     const double*   pk;
-    const Seg*      segs;
-    const Row*      rows;
     const BoxConst64* boxes;
-    unsigned int*   counter;
-    unsigned long long* out;
-    const unsigned int* range_keys;
-    uint32_t n_rows, n_items;
-    uint32_t n_bins;
-    uint32_t tj;
-    uint32_t smem_bins;
     double rmax, scale;         // r_max, n_bins / r_max
     BoxConst64 box0;            // PBOX variants (one box for all frames): the constants sit in the kernel-parameter
                                 // constant bank and are used as c[0x0][..] operands, no shared-memory loads
 };
-
-__host__ __device__ constexpr int tile_smem_bytes64(int smem_bins) {
-    return kSmemHeader + 2 * kStageBytes64 + (int)sizeof(BoxConst64) + 16 + 4 * (smem_bins + 2);
-}
 
 // ---- K0 for doubles ------------------------------------------------------------------------------
 struct RepackParams64 {
@@ -59,7 +46,7 @@ struct RepackParams64 {
     uint32_t blocks_per_frame;
 };
 
-__global__ void __launch_bounds__(256) repack_kernel_f64(const RepackParams64 P) {
+static __global__ void __launch_bounds__(256) repack_kernel_f64(const RepackParams64 P) {
     const uint32_t f = blockIdx.x / P.blocks_per_frame;
     const uint32_t slot = (blockIdx.x % P.blocks_per_frame) * blockDim.x + threadIdx.x;
     float fr[3] = {0.0f, 0.0f, 0.0f};
@@ -82,6 +69,7 @@ __global__ void __launch_bounds__(256) repack_kernel_f64(const RepackParams64 P)
                 for (int q = 0; q < 3; ++q) fr[q] = (float)(bc->Binv[3 * q] * x + bc->Binv[3 * q + 1] * y + bc->Binv[3 * q + 2] * z);
                 have = (fr[0] == fr[0]) && (fr[1] == fr[1]) && (fr[2] == fr[2]);
             }
+            if (!((x == x) && (y == y) && (z == z))) atomicOr(P.range_keys + 6, 1u);
         }
         double* g = P.pk + ((size_t)f * (P.frame_slots / kGroup) + slot / kGroup) * kGroupFloats + (slot % kGroup);
         g[0] = x; g[4] = y; g[8] = z;
@@ -152,157 +140,87 @@ __device__ __forceinline__ double pair_d2_f64(double xi, double yi, double zi, d
 }
 
 template <int MODE>
-__device__ __forceinline__ void bin_f64(double d2, double rmax, double scale, uint32_t last_bin, uint32_t hist,
-                                        uint32_t bin_lo, uint32_t lim, uint32_t trash, bool keep,
-                                        unsigned long long* __restrict__ grow) {
+__device__ __forceinline__ void bin_f64(double d2, double rmax, double scale, const HistView& hv, bool keep) {
     const double d = sqrt_rn_f64(d2);
     const uint32_t f = __double2uint_rd(__dmul_rn(d, scale));   // floor, saturating (one F2I)
-    const uint32_t b = min(f, last_bin) - bin_lo;               // reading Q3; unsigned wrap for bins below the sweep
+    const uint32_t bin = min(f, hv.last_bin);                   // reading Q3
+    const uint32_t b = bin - hv.lo;                             // unsigned wrap for bins below the sweep / window
     bool ok = keep && (d < rmax);                               // false for NaN (NaN input, +inf)
-    if constexpr (MODE == MODE_GLOBAL) { if (ok) atomicAdd(grow + b, 1ull); return; }    // bin_lo = 0 in this mode
-    if constexpr (MODE == MODE_SPLIT) ok = ok && b < lim;
-    hist_inc(ok ? hist + 4u * b : trash);
+    if constexpr (MODE == MODE_GLOBAL) { if (ok) atomicAdd(hv.grow + bin, 1ull); return; }
+    if constexpr (MODE == MODE_HYBRID) {
+        const bool in = ok && b < hv.lim;
+        hist_inc(in ? hv.hist_addr + 4u * b : hv.trash_addr);
+        if (ok && !in) atomicAdd(hv.grow + bin, 1ull);
+        return;
+    }
+    if constexpr (MODE == MODE_SPLIT) ok = ok && b < hv.lim;
+    hist_inc(ok ? hv.hist_addr + 4u * b : hv.trash_addr);
 }
 
-// ---- K1 for doubles: same schedule, stages and flush rule as tile_kernel (cdh_tile.cuh) ------------
-template <int BOX, int T, int MINB, bool PBOX, int MODE, bool SKIP = false>     // SKIP: as in cdh_tile.cuh
-__global__ void __launch_bounds__(T, MINB) tile_kernel_f64(const TileParams64 P) {
-    extern __shared__ __align__(128) unsigned char smem[];
-    constexpr int TI = T * kR;
-    uint64_t* bars = reinterpret_cast<uint64_t*>(smem);
-    volatile uint32_t* s_item = reinterpret_cast<volatile uint32_t*>(smem + 16);
-    double* stage0 = reinterpret_cast<double*>(smem + kSmemHeader);
-    BoxConst64* s_box = reinterpret_cast<BoxConst64*>(smem + kSmemHeader + 2 * kStageBytes64);
-    uint32_t* s_hist = reinterpret_cast<uint32_t*>(smem + kSmemHeader + 2 * kStageBytes64 + sizeof(BoxConst64) + 16);
-    const uint32_t hist_addr = smem_u32(s_hist);
-    const uint32_t bar_addr = smem_u32(bars);
-    const uint32_t stage_addr = smem_u32(stage0);
-    const int tid = threadIdx.x;
-
-    if (tid == 0) { mbar_init(bar_addr, 1); mbar_init(bar_addr + 8, 1); fence_mbar_init(); }
-    for (uint32_t b = tid; b <= P.smem_bins + 1; b += T) s_hist[b] = 0;
-    const uint32_t trash_addr = hist_addr + 4u * (P.smem_bins + 1u);
-    const bool range_ok = (BOX == BOX_TRI) ? (frac_range(P.range_keys) <= kPruneRange64) : true;
-    __syncthreads();
-
-    uint32_t stage_cnt = 0;
-    uint32_t cur_key = 0xFFFFFFFFu, cur_hist = 0, cur_lo = 0, cur_lim = 0, cur_box = 0xFFFFFFFFu;
-    uint64_t increments = 0;
-
-    auto flush = [&]() {
-        __syncthreads();
-        if (MODE != MODE_GLOBAL && cur_key != 0xFFFFFFFFu) {
-            unsigned long long* o = P.out + (size_t)cur_hist * P.n_bins;
-            for (uint32_t b = tid; b < cur_lim; b += T) {
-                const uint32_t v = s_hist[b];
-                if (v) { s_hist[b] = 0; atomicAdd(o + min(cur_lo + b, P.n_bins - 1u), (unsigned long long)v); }
-            }
-        }
-        increments = 0;
-        __syncthreads();
+// ---- the arithmetic policy of the double-precision tile kernel (cdh_sched.cuh) -----------------------
+template <int BOX, bool PBOX>
+struct MathF64 {
+    using Real = double;
+    using Box = BoxConst64;
+    using Params = TileParams64;
+    static constexpr int kStageBytes = kStageBytes64;
+    static constexpr bool kPeriodic = BOX != BOX_NONE;
+    static constexpr bool kHasClean = false;
+    static constexpr int kUnroll = 1;
+    struct Launch { bool range_ok; bool clean; };
+    struct Item {
+        double xi[4], yi[4], zi[4];
+        OrthoRegs64 ob;
+        bool prune;
     };
 
-    for (;;) {
-        if (tid == 0) *s_item = atomicAdd(P.counter, 1u);
-        __syncthreads();
-        const uint32_t item = *s_item;
-        if (item >= P.n_items) break;
-        uint32_t lo = 0, hi = P.n_rows;
-        while (hi - lo > 1) {
-            const uint32_t mid = (lo + hi) >> 1;
-            if (__ldg(&P.rows[mid].item_prefix) <= item) lo = mid; else hi = mid;
+    __device__ __forceinline__ static bool launch_begin(const Params& P, Launch& L) {
+        L.clean = false;
+        L.range_ok = (BOX == BOX_TRI) ? (frac_range(P.range_keys) <= kPruneRange64) : true;
+        return true;
+    }
+    template <int MODE>
+    __device__ __forceinline__ static void key_begin(const Params& P, const Launch&, const Seg& seg, HistView& hv) {
+        if constexpr (MODE == MODE_HYBRID) {
+            hv.lo = min(__ldg(P.win_lo + seg.hist), P.n_bins - min(P.n_bins, P.smem_bins));
+            hv.lim = min(P.smem_bins, P.n_bins - hv.lo);
+        } else {
+            hv.lo = seg.bin_lo; hv.lim = seg.bin_cnt + seg.last_sweep;
         }
-        const Row row = P.rows[lo];
-        const Seg seg = P.segs[row.seg];
-        const uint32_t jc = row.jc0 + (item - row.item_prefix);
-        const uint32_t j0 = jc * P.tj;
-        const uint32_t j1 = min((uint32_t)seg.nj, j0 + P.tj);
-        const uint32_t i0 = row.i0;
-
-        if (seg.key != cur_key || increments + (uint64_t)TI * P.tj > kMaxIncrements) {
-            flush();
-            cur_key = seg.key; cur_hist = seg.hist; cur_lo = seg.bin_lo;
-            cur_lim = seg.bin_cnt + seg.last_sweep;
-        }
-        increments += (uint64_t)TI * P.tj;
-        if (BOX != BOX_NONE && seg.box != cur_box) {
-            __syncthreads();
-            const double* src = reinterpret_cast<const double*>(P.boxes + seg.box);
-            for (int k = tid; k < (int)(sizeof(BoxConst64) / 8); k += T) reinterpret_cast<double*>(s_box)[k] = __ldg(src + k);
-            cur_box = seg.box;
-            __syncthreads();
-        }
-
-        // my R = 4 i-particles: one group of 12 doubles
-        const double2* gi = reinterpret_cast<const double2*>(P.pk + ((size_t)seg.i_group + (i0 >> 2) + tid) * kGroupFloats);
-        double xi[4], yi[4], zi[4];
-        { const double2 a = __ldg(gi), b = __ldg(gi + 1); xi[0] = a.x; xi[1] = a.y; xi[2] = b.x; xi[3] = b.y; }
-        { const double2 a = __ldg(gi + 2), b = __ldg(gi + 3); yi[0] = a.x; yi[1] = a.y; yi[2] = b.x; yi[3] = b.y; }
-        { const double2 a = __ldg(gi + 4), b = __ldg(gi + 5); zi[0] = a.x; zi[1] = a.y; zi[2] = b.x; zi[3] = b.y; }
-        const uint32_t ig = i0 + 4u * tid;
-        const uint32_t ig_warp = i0 + 4u * ((uint32_t)tid & ~31u);   // first i-particle of my warp
-        const bool warp_idle = ig_warp >= (uint32_t)seg.ni;          // my warp holds padding only
-
-        const bool masked = seg.same && (j0 < i0 + TI);
-        const uint32_t n_stage = (j1 - j0 + kStageParticles - 1) / kStageParticles;
-        const uint32_t s_begin = (masked && i0 > j0) ? (i0 - j0) / kStageParticles : 0;
-        const double* jsrc = P.pk + ((size_t)seg.j_group + (j0 >> 2)) * kGroupFloats;
-        const bool prune = (BOX == BOX_TRI) ? (range_ok && s_box->prune_ok != 0.0) : true;
-        unsigned long long* const grow = P.out + (size_t)seg.hist * P.n_bins;     // MODE_GLOBAL: the result row itself
-        OrthoRegs64 ob;
+    }
+    __device__ __forceinline__ static void item_begin(const Params&, const Launch& L, const double* __restrict__ g, const Box* s_box,
+                                                      const HistView&, Item& it) {
+        const double2* gi = reinterpret_cast<const double2*>(g);      // one group of 12 doubles
+        { const double2 a = __ldg(gi), b = __ldg(gi + 1); it.xi[0] = a.x; it.xi[1] = a.y; it.xi[2] = b.x; it.xi[3] = b.y; }
+        { const double2 a = __ldg(gi + 2), b = __ldg(gi + 3); it.yi[0] = a.x; it.yi[1] = a.y; it.yi[2] = b.x; it.yi[3] = b.y; }
+        { const double2 a = __ldg(gi + 4), b = __ldg(gi + 5); it.zi[0] = a.x; it.zi[1] = a.y; it.zi[2] = b.x; it.zi[3] = b.y; }
+        it.prune = (BOX == BOX_TRI) ? (L.range_ok && s_box->prune_ok != 0.0) : true;
         if constexpr (BOX == BOX_ORTHO) {
 #pragma unroll
-            for (int k = 0; k < 3; ++k) { ob.L[k] = s_box->L[k]; ob.invL[k] = s_box->invL[k]; }
+            for (int k = 0; k < 3; ++k) { it.ob.L[k] = s_box->L[k]; it.ob.invL[k] = s_box->invL[k]; }
         }
-
-        if (tid == 0 && s_begin < n_stage) {
-            const uint32_t b = stage_cnt & 1u;
-            mbar_expect_tx(bar_addr + 8 * b, kStageBytes64);
-            tma_load_1d(stage_addr + b * kStageBytes64, jsrc + (size_t)s_begin * kStageGroups * kGroupFloats, kStageBytes64, bar_addr + 8 * b);
-        }
-        for (uint32_t s = s_begin; s < n_stage; ++s) {
-            const uint32_t b = stage_cnt & 1u;
-            if (tid == 0 && s + 1 < n_stage) {
-                const uint32_t nb = b ^ 1u;
-                mbar_expect_tx(bar_addr + 8 * nb, kStageBytes64);
-                tma_load_1d(stage_addr + nb * kStageBytes64, jsrc + (size_t)(s + 1) * kStageGroups * kGroupFloats, kStageBytes64, bar_addr + 8 * nb);
-            }
-            mbar_wait(bar_addr + 8 * b, (stage_cnt >> 1) & 1u);
-            const double2* sj = reinterpret_cast<const double2*>(stage0 + b * (kStageBytes64 / 8));
-            const uint32_t jbase = j0 + s * kStageParticles;
-            const uint32_t n_grp = (SKIP && warp_idle) ? 0u : (min(j1 - jbase, (uint32_t)kStageParticles) + 3u) >> 2;
-            const bool stage_masked = masked && (jbase < i0 + TI);
-            // j-groups wholly below the diagonal for every lane of the warp are skipped, as is a padding-only warp
-            auto body = [&](auto masked_c, const uint32_t g_begin) {
-                constexpr bool MASKED = decltype(masked_c)::value;
-#pragma unroll 1
-                for (uint32_t g = g_begin; g < n_grp; ++g) {
-                    const uint32_t jg = jbase + 4u * g;
-#pragma unroll
-                    for (int h = 0; h < 2; ++h) {                   // two j-particles at a time (register pressure)
-                        const double2 XJ = sj[6 * g + h], YJ = sj[6 * g + 2 + h], ZJ = sj[6 * g + 4 + h];
-                        const double xj[2] = {XJ.x, XJ.y}, yj[2] = {YJ.x, YJ.y}, zj[2] = {ZJ.x, ZJ.y};
-#pragma unroll
-                        for (int c = 0; c < 2; ++c)
-#pragma unroll
-                            for (int r = 0; r < kR; ++r) {
-                                const bool keep = !MASKED || (jg + 2 * h + c > ig + r);
-                                double d2;
-                                if constexpr (PBOX) d2 = pair_d2_f64<BOX>(xi[r], yi[r], zi[r], xj[c], yj[c], zj[c], P.box0, ob, prune);
-                                else d2 = pair_d2_f64<BOX>(xi[r], yi[r], zi[r], xj[c], yj[c], zj[c], *s_box, ob, prune);
-                                bin_f64<MODE>(d2, P.rmax, P.scale, P.n_bins - 1u, hist_addr, cur_lo, cur_lim, trash_addr, keep, grow);
-                            }
-                    }
-                }
-            };
-            if (stage_masked) body(std::true_type{}, (SKIP && ig_warp > jbase) ? min(n_grp, (ig_warp - jbase) >> 2) : 0u);
-            else body(std::false_type{}, 0u);
-            __syncthreads();
-            ++stage_cnt;
-        }
-        __syncthreads();
     }
-    flush();
-}
+    template <int MODE, int KIND>
+    __device__ __forceinline__ static void group(const Params& P, const Launch&, const Item& it, const unsigned char* stage,
+                                                 uint32_t g, uint32_t jg, uint32_t ig, const HistView& hv, const Box* s_box) {
+        constexpr bool MASKED = KIND == KIND_MASKED;
+        const double2* sj = reinterpret_cast<const double2*>(stage);
+#pragma unroll
+        for (int h = 0; h < 2; ++h) {                   // two j-particles at a time (register pressure)
+            const double2 XJ = sj[6 * g + h], YJ = sj[6 * g + 2 + h], ZJ = sj[6 * g + 4 + h];
+            const double xj[2] = {XJ.x, XJ.y}, yj[2] = {YJ.x, YJ.y}, zj[2] = {ZJ.x, ZJ.y};
+#pragma unroll
+            for (int c = 0; c < 2; ++c)
+#pragma unroll
+                for (int r = 0; r < kR; ++r) {
+                    const bool keep = !MASKED || (jg + 2 * h + c > ig + r);
+                    double d2;
+                    if constexpr (PBOX) d2 = pair_d2_f64<BOX>(it.xi[r], it.yi[r], it.zi[r], xj[c], yj[c], zj[c], P.box0, it.ob, it.prune);
+                    else d2 = pair_d2_f64<BOX>(it.xi[r], it.yi[r], it.zi[r], xj[c], yj[c], zj[c], *s_box, it.ob, it.prune);
+                    bin_f64<MODE>(d2, P.rmax, P.scale, hv, keep);
+                }
+        }
+    }
+};
 
 }  // namespace cdh

@@ -10,7 +10,7 @@
 // VAR_FAST computes the same integers with packed f32x2 arithmetic, a magic-number rint/floor, a
 // Newton-corrected MUFU.RSQ square root and a threshold on d2.
 #pragma once
-#include "cdh_device.cuh"
+#include "cdh_sched.cuh"
 
 namespace cdh {
 
@@ -23,10 +23,6 @@ constexpr int VAR_SIMPLE_MATCH = 2;
 constexpr int VAR_SIMPLE_PLAIN = 3;
 
 constexpr int BOX_NONE = 0, BOX_ORTHO = 1, BOX_TRI = 2;
-
-// Where the histogram lives: one shared-memory copy of all bins; a shared copy of one bin range per sweep; no private
-// copy at all, updates go straight to the uint64 result in L2 (very wide histograms).
-constexpr int MODE_SHARED = 0, MODE_SPLIT = 1, MODE_GLOBAL = 2;
 
 // Triclinic zero structure (skipping a term whose matrix entry is exactly 0 in B and in B^-1 changes
 // at most the sign of a zero, never d2): 0 general 3x3, 1 upper triangular (a along x, b in the xy
@@ -47,8 +43,9 @@ struct RepackParams {
     float* pk;                  // [n_frames][frame_groups][12]
     const int32_t* off;         // device, [n_species+1] particle offsets
     const uint32_t* pad_off;    // device, [n_species+1] padded particle offsets (multiples of kPadParticles)
-    unsigned int* range_keys;   // device, [6]: atomicMax of key(f_k) (k = 0..2) and of ~key(f_k) (3..5), f = b^-1 x
-                                // (fractional coordinates, approximate); zero-initialised; see frac_range()
+    unsigned int* range_keys;   // device, [7]: atomicMax of key(f_k) (k = 0..2) and of ~key(f_k) (3..5), f = b^-1 x
+                                // (fractional coordinates, approximate; the raw coordinates when there is no box), [6] is set
+                                // when a particle has a NaN coordinate; zero-initialised; see frac_range() / coord_extent2_ru()
     const BoxConst* boxes;      // box constants (periodic boxes), one or n_frames
     int32_t n_species, n_total, n_frames;
     int32_t box_type, n_boxes;
@@ -82,7 +79,24 @@ __device__ __forceinline__ float frac_range(const unsigned int* __restrict__ key
     return r;
 }
 
-__global__ void __launch_bounds__(256) repack_kernel(const RepackParams P) {
+// No box: an UPPER bound of every pinned d2 of the call, sum over the axes of (max - min)^2 with every operation rounded
+// up (subtraction, square and sum are monotone, so the round-to-nearest d2 of any pair is below it).  +inf when a
+// particle has a NaN coordinate; 0 when there are no particles.
+__device__ __forceinline__ float coord_extent2_ru(const unsigned int* __restrict__ keys) {
+    if (__ldg(keys + 6) != 0u) return __int_as_float(0x7f800000);
+    float acc = 0.0f;
+#pragma unroll
+    for (int q = 0; q < 3; ++q) {
+        const uint32_t kmax = __ldg(keys + q), kmin_c = __ldg(keys + 3 + q);
+        if (kmax != 0u) {
+            const float ext = __fsub_ru(key_float(kmax), key_float(~kmin_c));
+            acc = __fadd_ru(acc, __fmul_ru(ext, ext));
+        }
+    }
+    return acc;
+}
+
+static __global__ void __launch_bounds__(256) repack_kernel(const RepackParams P) {
     const uint32_t f = blockIdx.x / P.blocks_per_frame;
     const uint32_t slot = (blockIdx.x % P.blocks_per_frame) * blockDim.x + threadIdx.x;
     float fr[3] = {0.0f, 0.0f, 0.0f};
@@ -111,13 +125,17 @@ __global__ void __launch_bounds__(256) repack_kernel(const RepackParams P) {
 #pragma unroll
                 for (int q = 0; q < 3; ++q) fr[q] = bc->Binv[3 * q] * x + bc->Binv[3 * q + 1] * y + bc->Binv[3 * q + 2] * z;
                 have = true;
+            } else {
+                fr[0] = x; fr[1] = y; fr[2] = z;            // no box: the extent of the coordinates themselves
+                have = true;
             }
             have = have && (fr[0] == fr[0]) && (fr[1] == fr[1]) && (fr[2] == fr[2]);
+            if (!((x == x) && (y == y) && (z == z))) atomicOr(P.range_keys + 6, 1u);   // rare: a NaN input coordinate
         }
         float* g = P.pk + ((size_t)f * (P.frame_slots / kGroup) + slot / kGroup) * kGroupFloats + (slot % kGroup);
         g[0] = x; g[4] = y; g[8] = z;
     }
-    if (P.box_type != BOX_NONE) {
+    {
         // CTA max / min of the order-preserving keys (shared atomics), then one global atomic per key and CTA
         __shared__ unsigned int s_keys[6];
         if (threadIdx.x < 6) s_keys[threadIdx.x] = 0u;
@@ -133,6 +151,83 @@ __global__ void __launch_bounds__(256) repack_kernel(const RepackParams P) {
         }
         __syncthreads();
         if (threadIdx.x < 6 && s_keys[threadIdx.x] != 0u) atomicMax(P.range_keys + threadIdx.x, s_keys[threadIdx.x]);
+    }
+}
+
+// ---------------------------------------------------------------------------------------------
+// K0b: window_kernel (MODE_HYBRID, very wide histograms).  One CTA per histogram row samples pairs of the row's first
+// segment, bins their APPROXIMATE distances (plain float arithmetic, Eq. 5 without the neighbour search) into 1024
+// coarse cells and writes the first bin of the `window` consecutive bins that hold the most samples: the tile kernel
+// keeps that window of the row in shared memory and sends the rest to L2.  The choice only affects speed, never the
+// result, so nothing here belongs to the pinned sequence.
+// ---------------------------------------------------------------------------------------------
+constexpr int kWindowCells = 1024;
+constexpr int kWindowSamplesPerThread = 64;
+
+template <class Real, class Box>
+struct WindowParams {
+    const Real* pk;
+    const Seg* segs;
+    const int32_t* row_seg;     // [n_hist] first segment of each histogram row, -1 if the row has no pairs
+    const Box* boxes;
+    uint32_t* win_lo;           // [n_hist] out
+    int32_t box_type;
+    uint32_t n_bins, window;    // window: bins the shared histogram holds
+    float scale;                // n_bins / r_max
+};
+
+__device__ __forceinline__ uint32_t window_hash(uint32_t x) {
+    x ^= x >> 16; x *= 0x7feb352du; x ^= x >> 15; x *= 0x846ca68bu; x ^= x >> 16;
+    return x;
+}
+
+template <class Real, class Box>
+__global__ void __launch_bounds__(256) window_kernel(const WindowParams<Real, Box> P) {
+    __shared__ uint32_t cells[kWindowCells];
+    __shared__ uint32_t best_lo;
+    for (int k = threadIdx.x; k < kWindowCells; k += 256) cells[k] = 0;
+    __syncthreads();
+    const int32_t sid = __ldg(P.row_seg + blockIdx.x);
+    if (sid < 0) { if (threadIdx.x == 0) P.win_lo[blockIdx.x] = 0; return; }
+    const Seg seg = P.segs[sid];
+    const Box* bc = P.boxes + seg.box;
+    auto coord = [&](uint32_t group0, uint32_t k, float (&x)[3]) {
+        const Real* g = P.pk + ((size_t)group0 + (k >> 2)) * kGroupFloats + (k & 3u);
+        x[0] = (float)g[0]; x[1] = (float)g[4]; x[2] = (float)g[8];
+    };
+    for (int s = 0; s < kWindowSamplesPerThread; ++s) {
+        const uint32_t h = window_hash((blockIdx.x * 256u + threadIdx.x) * kWindowSamplesPerThread + s + 0x9e3779b9u);
+        const uint32_t i = __umulhi(h, (uint32_t)seg.ni), j = __umulhi(window_hash(h ^ 0x85ebca6bu), (uint32_t)seg.nj);
+        float a[3], b[3], d[3];
+        coord(seg.i_group, i, a); coord(seg.j_group, j, b);
+#pragma unroll
+        for (int c = 0; c < 3; ++c) d[c] = b[c] - a[c];
+        if (P.box_type == BOX_ORTHO) {
+#pragma unroll
+            for (int c = 0; c < 3; ++c) d[c] -= (float)bc->L[c] * rintf(d[c] * (float)bc->invL[c]);
+        } else if (P.box_type == BOX_TRI) {
+            float n[3];
+#pragma unroll
+            for (int k = 0; k < 3; ++k) n[k] = rintf((float)bc->Binv[3 * k] * d[0] + (float)bc->Binv[3 * k + 1] * d[1] + (float)bc->Binv[3 * k + 2] * d[2]);
+#pragma unroll
+            for (int c = 0; c < 3; ++c) d[c] -= (float)bc->B[3 * c] * n[0] + (float)bc->B[3 * c + 1] * n[1] + (float)bc->B[3 * c + 2] * n[2];
+        }
+        const float t = sqrtf(d[0] * d[0] + d[1] * d[1] + d[2] * d[2]) * P.scale;      // NaN / out of range: not counted
+        if (t >= 0.0f && t < (float)P.n_bins)
+            atomicAdd(&cells[min((uint32_t)(t * ((float)kWindowCells / (float)P.n_bins)), (uint32_t)kWindowCells - 1u)], 1u);
+    }
+    __syncthreads();
+    if (threadIdx.x == 0) {
+        // sliding window of w cells over the coarse histogram; the first maximum wins
+        const uint32_t w = max(1u, (uint32_t)(((uint64_t)P.window * kWindowCells) / P.n_bins));
+        uint32_t sum = 0, best = 0, lo = 0;
+        for (uint32_t c = 0; c < (uint32_t)kWindowCells; ++c) {
+            sum += cells[c];
+            if (c >= w) sum -= cells[c - w];
+            if (sum > best) { best = sum; lo = c + 1 >= w ? c + 1 - w : 0; }
+        }
+        best_lo = (uint32_t)(((uint64_t)lo * P.n_bins) / kWindowCells);
+        P.win_lo[blockIdx.x] = min(best_lo, P.n_bins - min(P.n_bins, P.window));
     }
 }
 

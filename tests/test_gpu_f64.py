@@ -208,8 +208,16 @@ def test_f64_wide_histogram_global_and_split():
     p = inputs.uniform_problem(19, (4000,), inputs.BOX_NONE, 800_000, math.sqrt(3.0))
     want = oracle64(p)
     a, info = gpu64(p)
+    assert info["hybrid"] and info["sweeps"] == 1             # a shared window of the bins + L2 updates, one sweep
+    same(a, want, f"f64 800k bins, hybrid window {info}")
+    g, info = gpu64(p, cdh.FLAG_GLOBAL_HIST)
     assert info["global_hist"] and info["sweeps"] == 1
-    same(a, want, f"f64 800k bins, global histogram {info}")
+    same(g, want, f"f64 800k bins, global histogram {info}")
+    for nb in (60_000, 100_000, 200_000):                     # the bin counts just above one CTA's shared memory
+        q = inputs.uniform_problem(23, (3000, 2000), inputs.BOX_ORTHO, nb, 3.0, box=np.diag([6.0, 7.0, 8.0]))
+        h, info = gpu64(q)
+        assert info["hybrid"] and info["sweeps"] == 1
+        same(h, oracle64(q), f"f64 {nb} bins orthorhombic, hybrid window {info}")
     b, info = gpu64(p, 45000 << cdh.FLAG_MAX_SMEM_BINS_SHIFT)
     assert not info["global_hist"] and info["sweeps"] == 18
     same(b, want, f"f64 800k bins, 18 sweeps {info}")

@@ -212,8 +212,8 @@ def test_p8_single_bin_exceeds_uint32():
 
 
 def test_p9_wide_histogram_global_and_split_paths():
-    # 1,000,000 bins = 4 MB >> shared memory: the global-histogram mode takes over by itself; a cap on the shared
-    # bins forces the bin-range-split path (20 sweeps) instead; both must equal the oracle
+    # 1,000,000 bins = 4 MB >> shared memory: beyond 16 shared windows the global-histogram mode takes over by itself;
+    # a cap on the shared bins forces the bin-range-split path (20 sweeps) instead; both must equal the oracle
     p = inputs.uniform_problem(9, (6000,), inputs.BOX_NONE, 1_000_000, math.sqrt(3.0))
     got, info = gpu_hist(p)
     assert info["global_hist"] and info["sweeps"] == 1
@@ -223,8 +223,32 @@ def test_p9_wide_histogram_global_and_split_paths():
     assert_same(got, oracle_hist(p), f"1M bins, 20 sweeps {info}")
     q = inputs.uniform_problem(10, (2500, 3000), inputs.BOX_ORTHO, 400_000, 3.0, box=np.diag([6.0, 7.0, 8.0]))
     got, info = gpu_hist(q)
+    assert info["hybrid"] and info["sweeps"] == 1
+    assert_same(got, oracle_hist(q), f"400k bins orthorhombic, hybrid window {info}")
+    got, info = gpu_hist(q, cdh.FLAG_GLOBAL_HIST)
     assert info["global_hist"]
-    assert_same(got, oracle_hist(q), f"400k bins orthorhombic, global histogram {info}")
+    assert_same(got, oracle_hist(q), f"400k bins orthorhombic, forced global histogram {info}")
+
+
+@pytest.mark.parametrize("n_bins", [56_000, 60_000, 100_000, 200_000])
+@pytest.mark.parametrize("box_type", [inputs.BOX_NONE, inputs.BOX_ORTHO, inputs.BOX_TRICLINIC])
+def test_hybrid_window_single_sweep(n_bins, box_type):
+    """Bin counts just above what one CTA's shared memory holds (the paper's staircase of sweeps,
+    PAPER.md:205, 308-316): one sweep with the most populated window of every row in shared memory and the rest in L2.
+    Several species, so that every row picks its own window; also a clustered set (config-5 recipe), whose first bins
+    are far more populated than a uniform set's."""
+    box = {inputs.BOX_NONE: None, inputs.BOX_ORTHO: np.diag([5.0, 6.0, 7.0]),
+           inputs.BOX_TRICLINIC: np.array([[6.0, 0.0, 0.0], [1.0, 5.5, 0.0], [-0.5, 1.5, 5.0]])}[box_type]
+    r_max = 9.0 if box_type == inputs.BOX_NONE else 2.4
+    p = inputs.uniform_problem(n_bins + box_type, (2100, 4200, 900), box_type, n_bins, r_max, box=box, spread=5.0 if box_type == inputs.BOX_NONE else 1.0)
+    got, info = gpu_hist(p)
+    assert info["sweeps"] == 1 and info["hybrid"] == (n_bins > 56_402), info
+    assert_same(got, oracle_hist(p), f"{n_bins} bins, box {box_type}: {info}")
+    if box_type == inputs.BOX_NONE:
+        c = inputs.config5(n=12_000, n_bins=n_bins, n_clusters=25)
+        got, info = gpu_hist(c)
+        assert_same(got, oracle_hist(c), f"{n_bins} bins, clustered set: {info}")
+        assert int(got.sum()) == 12_000 * 11_999 // 2
 
 
 def test_empty_species_tiny_inputs_and_nan():
