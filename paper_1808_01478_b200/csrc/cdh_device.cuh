@@ -136,6 +136,10 @@ __device__ __forceinline__ void hist_inc(uint32_t addr) {
 __device__ __forceinline__ void hist_inc_if(bool keep, uint32_t addr) {
     asm volatile("{\n.reg .pred p;\nsetp.ne.u32 p, %1, 0;\n@p red.shared.add.u32 [%0], 1;\n}\n" ::"r"(addr), "r"((uint32_t)keep) : "memory");
 }
+// Global uint64 counter += 1 under a predicate, no return value (SASS: @P REDG.E.ADD.64): no branch around the reduction.
+__device__ __forceinline__ void red_global_inc_if(bool keep, unsigned long long* addr) {
+    asm volatile("{\n.reg .pred p;\nsetp.ne.u32 p, %1, 0;\n@p red.global.add.u64 [%0], 1;\n}\n" ::"l"(addr), "r"((uint32_t)keep) : "memory");
+}
 __device__ __forceinline__ void hist_add(uint32_t addr, uint32_t v) {
     asm volatile("red.shared.add.u32 [%0], %1;" ::"r"(addr), "r"(v) : "memory");
 }

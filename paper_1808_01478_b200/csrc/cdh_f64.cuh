@@ -146,11 +146,11 @@ __device__ __forceinline__ void bin_f64(double d2, double rmax, double scale, co
     const uint32_t bin = min(f, hv.last_bin);                   // reading Q3
     const uint32_t b = bin - hv.lo;                             // unsigned wrap for bins below the sweep / window
     bool ok = keep && (d < rmax);                               // false for NaN (NaN input, +inf)
-    if constexpr (MODE == MODE_GLOBAL) { if (ok) atomicAdd(hv.grow + bin, 1ull); return; }
+    if constexpr (MODE == MODE_GLOBAL) { red_global_inc_if(ok, hv.grow + bin); return; }
     if constexpr (MODE == MODE_HYBRID) {
         const bool in = ok && b < hv.lim;
         hist_inc(in ? hv.hist_addr + 4u * b : hv.trash_addr);
-        if (ok && !in) atomicAdd(hv.grow + bin, 1ull);
+        red_global_inc_if(ok && !in, hv.grow + bin);
         return;
     }
     if constexpr (MODE == MODE_SPLIT) ok = ok && b < hv.lim;

@@ -8,6 +8,10 @@
 #pragma once
 #include "cdh_fast.cuh"
 
+#ifndef CDH_ONE_U
+#define CDH_ONE_U 1     // 1: the second opaque 1.0f (TileParams::one_u) lives in a uniform register
+#endif
+
 namespace cdh {
 
 struct ItemF32 {
@@ -48,6 +52,8 @@ struct MathFast {
     struct Item : ItemF32 {
         FastBox fb;
         uint32_t addr_c, sub_c;
+        unsigned long long* grow;   // the result row, pinned in a register pair (MODE_GLOBAL / MODE_HYBRID): ptxas otherwise
+                                    // rebuilds it from (out, row, n_bins) next to every reduction
     };
 
     __device__ __forceinline__ static bool launch_begin(const Params& P, Launch& L) {
@@ -64,7 +70,7 @@ struct MathFast {
         } else {
             L.clean = __float_as_uint(coord_extent2_ru(P.range_keys)) < P.thr2_bits;
         }
-        L.ones.r = dup2(P.one); L.ones.u = dup2(P.one_u);
+        L.ones.r = dup2(P.one); L.ones.u = CDH_ONE_U ? dup2(P.one_u) : L.ones.r;
         L.scale = dup2(P.scale);
         return true;
     }
@@ -92,13 +98,14 @@ struct MathFast {
         }
         it.addr_c = hv.hist_addr - 4u * (kFloorMagicBits + hv.lo);
         it.sub_c = kFloorMagicBits + hv.lo;
+        asm volatile("mov.b64 %0, %1;" : "=l"(it.grow) : "l"(hv.grow));
     }
 
     template <int MODE, int KIND>
     __device__ __forceinline__ static void group(const Params& P, const Launch& L, const Item& it, const unsigned char* stage,
                                                  uint32_t g, uint32_t jg, uint32_t ig, const HistView& hv, const Box* s_box) {
         constexpr bool MASKED = KIND == KIND_MASKED;
-        constexpr bool CLEAN = KIND == KIND_CLEAN && MODE == MODE_SHARED;
+        constexpr bool CLEAN = KIND == KIND_CLEAN && (MODE == MODE_SHARED || MODE == MODE_HYBRID || MODE == MODE_GLOBAL);
         const float4* sj = reinterpret_cast<const float4*>(stage);
         const float4 XJ = sj[3 * g], YJ = sj[3 * g + 1], ZJ = sj[3 * g + 2];
         const f2 XA = pk2(XJ.x, XJ.y), XB = pk2(XJ.z, XJ.w), YA = pk2(YJ.x, YJ.y), YB = pk2(YJ.z, YJ.w),
@@ -150,7 +157,7 @@ struct MathFast {
             for (int hlf = 0; hlf < 2; ++hlf) {
                 bool k0 = true, k1 = true;
                 if constexpr (MASKED) { k0 = jg + 2 * hlf > ig + r; k1 = jg + 2 * hlf + 1 > ig + r; }
-                bin_fast2<MODE, CLEAN>(D2[r][hlf], k0, k1, L.scale, L.ones.r, P.thr2_bits, it.addr_c, it.sub_c, hv);
+                bin_fast2<MODE, CLEAN>(D2[r][hlf], k0, k1, L.scale, L.ones.r, P.thr2_bits, it.addr_c, it.sub_c, hv, it.grow);
             }
         }
     }
