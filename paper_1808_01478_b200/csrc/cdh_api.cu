@@ -138,6 +138,7 @@ bool small_species(const int32_t* off, int32_t n_species) {
 #define CDH_ITEMS_PER_CTA 64   // work items per resident CTA the j-chunk size is shrunk for (tail of the dynamic schedule)
 #endif
 constexpr uint64_t kItemsPerCta = CDH_ITEMS_PER_CTA;
+constexpr uint32_t kMinChunk = 32;     // smallest j-chunk (particles)
 #ifndef CDH_STAGES
 #define CDH_STAGES 4           // stages of the TMA ring (cdh_sched.cuh) when the private histogram leaves the room; else 2
 #endif
@@ -419,7 +420,10 @@ int build_plan(cdh_ctx* ctx, cudaStream_t stream, int32_t n_frames, const int32_
     uint32_t tj = 8192;
     for (;; tj >>= 1) {
         build_tables(n_frames, off, n_species, nb > 0 ? nb : 1, (uint32_t)n_bins, sp, ti, tj, pad_off, frame_slots, &wt);
-        if (wt.n_items >= kItemsPerCta * grid_full || tj == (uint32_t)kStageParticles) break;
+        if (wt.n_items >= kItemsPerCta * grid_full) break;
+        // small calls: j-chunks below one stage (the stage is then partly used) until every resident CTA has an item --
+        // a 2,000-particle frame becomes 94 items of 1024 x 32 pairs instead of 12 of 1024 x 256 (launch-latency regime)
+        if (tj <= (uint32_t)kStageParticles && (wt.n_items >= grid_full || tj == kMinChunk)) break;
     }
     if (wt.n_items >= 0xffffffffull || wt.rows.size() >= 0x7fffffffull) return CDH_ERR_INVALID_ARG;
     std::vector<int32_t> row_seg((size_t)n_hist, -1);          // first segment of each histogram row (window_kernel)
@@ -502,8 +506,11 @@ int enqueue_plan(cdh_ctx* ctx, const Plan& pl, const void* coords, cudaStream_t 
     if (stream != pl.up_stream) CDH_CUDA(cudaStreamWaitEvent(stream, pl.uploaded, 0));   // the tables went up on another stream
     if (timing) CDH_CUDA(cudaEventRecord(ev[0], stream));
     CDH_CUDA(cudaMemsetAsync(ctx->d_scalars, 0, 64, stream));
-    if (!(ctx->flags & CDH_FLAG_ACCUMULATE))
-        CDH_CUDA(cudaMemsetAsync(out, 0, (size_t)pl.n_hist * (size_t)pl.n_bins * sizeof(uint64_t), stream));
+    const bool zero_out = !(ctx->flags & CDH_FLAG_ACCUMULATE);
+    const uint64_t out_count = (uint64_t)pl.n_hist * (uint64_t)pl.n_bins;
+    // the repack kernel zeroes the result on its way unless that would be most of its work (few particles, very many bins)
+    const bool fold_zero = zero_out && pl.frame_slots > 0 && out_count <= 64ull * 256ull * pl.repack_blocks;
+    if (zero_out && !fold_zero) CDH_CUDA(cudaMemsetAsync(out, 0, out_count * sizeof(uint64_t), stream));
 
     // ---- K0 repack -----------------------------------------------------------------------------
     if (pl.frame_slots > 0) {
@@ -515,6 +522,7 @@ int enqueue_plan(cdh_ctx* ctx, const Plan& pl, const void* coords, cudaStream_t 
             rp.n_species = pl.n_species; rp.n_total = pl.n_total; rp.n_frames = pl.n_frames;
             rp.box_type = pl.box_type; rp.n_boxes = pl.n_boxes;
             rp.frame_slots = pl.frame_slots; rp.blocks_per_frame = pl.blocks_per_frame;
+            rp.zero = fold_zero ? (unsigned long long*)out : nullptr; rp.zero_count = out_count;
             repack_kernel_f64<<<pl.repack_blocks, 256, 0, stream>>>(rp);
         } else {
             RepackParams rp;
@@ -524,6 +532,7 @@ int enqueue_plan(cdh_ctx* ctx, const Plan& pl, const void* coords, cudaStream_t 
             rp.n_species = pl.n_species; rp.n_total = pl.n_total; rp.n_frames = pl.n_frames;
             rp.box_type = pl.box_type; rp.n_boxes = pl.n_boxes;
             rp.frame_slots = pl.frame_slots; rp.blocks_per_frame = pl.blocks_per_frame;
+            rp.zero = fold_zero ? (unsigned long long*)out : nullptr; rp.zero_count = out_count;
             repack_kernel<<<pl.repack_blocks, 256, 0, stream>>>(rp);
         }
         CDH_CUDA(cudaGetLastError());
@@ -739,8 +748,8 @@ extern "C" int cdh_host_fused_rint_constant(float inv_l, float* inv_lf) {
 
 extern "C" int64_t cdh_host_work_items(int32_t n_frames, const int32_t* off, int32_t n_species, int32_t n_bins,
                                        int32_t cap_bins, int32_t ti, int32_t tj, int64_t* items, int64_t max_items) {
-    if (!off || n_frames < 1 || n_species < 1 || n_bins < 1 || cap_bins < 1 || ti < 4 || tj < kStageParticles ||
-        tj % kStageParticles || (max_items > 0 && !items))
+    if (!off || n_frames < 1 || n_species < 1 || n_bins < 1 || cap_bins < 1 || ti < 4 || tj < (int32_t)kMinChunk ||
+        tj % (int32_t)kMinChunk || (tj > kStageParticles && tj % kStageParticles) || (max_items > 0 && !items))
         return -1;
     std::vector<uint32_t> pad_off((size_t)n_species + 1);
     uint64_t slots = 0;

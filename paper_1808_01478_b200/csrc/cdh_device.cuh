@@ -75,7 +75,7 @@ struct TileCommon {
     const uint32_t* win_lo;     // MODE_HYBRID: first bin of the shared-memory window of each histogram row (device; window_kernel)
     uint32_t n_rows, n_items;
     uint32_t n_bins;
-    uint32_t tj;                // j-chunk size in particles (multiple of kStageParticles)
+    uint32_t tj;                // j-chunk size in particles (a multiple of kStageParticles, or 32 / 64 / 128 for small calls)
     uint32_t smem_bins;         // capacity of the shared histogram (bins per sweep / window, without the two extra slots)
     uint32_t n_stages;          // stages of the TMA ring (power of two, 2..8)
 };

@@ -44,9 +44,13 @@ struct RepackParams64 {
     int32_t box_type, n_boxes;
     uint32_t frame_slots;
     uint32_t blocks_per_frame;
+    unsigned long long* zero;   // as RepackParams
+    uint64_t zero_count;
 };
 
 static __global__ void __launch_bounds__(256) repack_kernel_f64(const RepackParams64 P) {
+    if (P.zero != nullptr)
+        for (uint64_t k = (uint64_t)blockIdx.x * 256u + threadIdx.x; k < P.zero_count; k += (uint64_t)gridDim.x * 256u) P.zero[k] = 0ull;
     const uint32_t f = blockIdx.x / P.blocks_per_frame;
     const uint32_t slot = (blockIdx.x % P.blocks_per_frame) * blockDim.x + threadIdx.x;
     float fr[3] = {0.0f, 0.0f, 0.0f};

@@ -51,6 +51,8 @@ struct RepackParams {
     int32_t box_type, n_boxes;
     uint32_t frame_slots;       // padded particles per frame
     uint32_t blocks_per_frame;
+    unsigned long long* zero;   // the call's result, zeroed here (grid-stride) unless the call accumulates: nullptr then
+    uint64_t zero_count;        // uint64 elements of it
 };
 
 // Order-preserving map float -> uint32 (never 0 for a non-NaN float except -NaN patterns, which are excluded).
@@ -97,6 +99,8 @@ __device__ __forceinline__ float coord_extent2_ru(const unsigned int* __restrict
 }
 
 static __global__ void __launch_bounds__(256) repack_kernel(const RepackParams P) {
+    if (P.zero != nullptr)      // saves the call one memset node (small calls are launch-latency bound)
+        for (uint64_t k = (uint64_t)blockIdx.x * 256u + threadIdx.x; k < P.zero_count; k += (uint64_t)gridDim.x * 256u) P.zero[k] = 0ull;
     const uint32_t f = blockIdx.x / P.blocks_per_frame;
     const uint32_t slot = (blockIdx.x % P.blocks_per_frame) * blockDim.x + threadIdx.x;
     float fr[3] = {0.0f, 0.0f, 0.0f};

@@ -77,7 +77,7 @@ def covered_pairs(items, ni, nj, same, ti):
 
 
 @pytest.mark.parametrize("counts,ti,tj", [((700,), 256, 256), ((1030, 517), 1024, 256), ((5, 0, 2100, 1), 1024, 512),
-                                          ((3000,), 4096, 1024)])
+                                          ((3000,), 4096, 1024), ((2000,), 1024, 32), ((700, 130), 1024, 64)])
 def test_work_list_covers_every_pair_exactly_once(lib, counts, ti, tj):
     off = np.concatenate([[0], np.cumsum(counts)]).astype(np.int32)
     n_species, n_frames, n_bins, cap = len(counts), 2, 1000, 300            # 4 sweeps
