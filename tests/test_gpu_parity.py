@@ -278,7 +278,7 @@ def test_sqrt_selftest_sample():
     _need_gpu()
     # full range is bench.py --selftest; here 2^26 patterns around 1.0 and the low end of the range
     assert cdh.cdh_selftest_sqrt(0x3F000000, 0x3F000000 + (1 << 26)) == 0
-    assert cdh.cdh_selftest_sqrt(0x0D000000, 0x0D000000 + (1 << 24)) == 0
+    assert cdh.cdh_selftest_sqrt(0x0D800000, 0x0D800000 + (1 << 24)) == 0
 
 
 def test_argument_errors_leave_out_untouched():
