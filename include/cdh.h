@@ -43,7 +43,7 @@ extern "C" {
 /* return codes */
 #define CDH_OK                 0
 #define CDH_ERR_INVALID_ARG  (-1)  /* detected before anything is enqueued; out untouched */
-#define CDH_ERR_UNSUPPORTED  (-2)
+#define CDH_ERR_UNSUPPORTED  (-2)  /* the library was built without the kernel variant the call needs (nothing enqueued) */
 #define CDH_ERR_ALLOC        (-3)  /* device or pinned-host allocation failed */
 #define CDH_ERR_CUDA         (-4)  /* a CUDA runtime call failed; text via cdh_last_error() */
 
@@ -57,9 +57,11 @@ extern "C" {
 #define CDH_FLAG_NO_AGGREGATE    (1u << 3) /* plain kernel, one ATOMS.ADD per lane (no aggregation at all);
                                               production uses ATOMS.POPC.INC, which merges equal addresses in hardware */
 #define CDH_FLAG_TIME_KERNELS     (1u << 4) /* record CUDA events around the tile kernel(s) of every call
-                                              (measurement; read with cdh_last_call_kernel_ms) */
+                                              (measurement; read with cdh_call_kernel_ms) */
 #define CDH_FLAG_GLOBAL_HIST      (1u << 5) /* no private histogram: every kept pair adds to the uint64 result
-                                              directly (chosen automatically for very wide histograms) */
+                                              directly (chosen automatically beyond 16 shared-memory windows of bins;
+                                              between one and 16 windows the library keeps the most populated window of
+                                              every histogram row in shared memory and sends the rest to L2, in one sweep) */
 #define CDH_FLAG_ACCUMULATE       (1u << 6) /* cdh_histograms ADDS to `out` instead of overwriting it: a caller can feed a
                                               trajectory in chunks of frames (the paper's writer sums every 100 frames,
                                               PAPER.md:338).  Not for cdh_histograms_host (its device result is scratch) */
@@ -83,7 +85,7 @@ int cdh_create(cdh_ctx **ctx, int device, uint32_t flags);
  *  n_frames        >= 1.
  *  species_offsets HOST pointer, [n_species + 1]; [0] == 0, non-decreasing, [n_species] == n_total < 2^31;
  *                  the same for every frame.  Empty species are legal (zero histograms).
- *  n_species       >= 1.
+ *  n_species       1 .. 4096 (the work tables hold one row of segments per species pair and frame).
  *  box_type        CDH_BOX_*.
  *  box             HOST pointer, [n_boxes][9] row-major doubles, ROWS are the box vectors a, b, c
  *                  (the mathematical b of Eq. 5 has them as columns); NULL iff CDH_BOX_NONE.
@@ -94,14 +96,26 @@ int cdh_create(cdh_ctx **ctx, int device, uint32_t flags);
  *  n_bins          1 .. 2^22.  Bin width r_max / n_bins; bin = floor(r * (float)(n_bins / r_max)),
  *                  a kept pair whose product rounds up to n_bins goes to bin n_bins - 1.
  *  precision       CDH_F32 or CDH_F64 (constants are then used in double: r_max, n_bins / r_max, the box).
- *  stream          cudaStream_t (as void*), may be 0.  All work is enqueued on it; the call does not
- *                  synchronise.  `out` is valid once the caller has synchronised the stream.
+ *  stream          cudaStream_t (as void*), may be 0.  All device work is enqueued on it and `out` is valid once the
+ *                  caller has synchronised the stream.  What the HOST does depends on whether the context has seen
+ *                  these arguments before (everything but the coords / out pointers and the accumulate flag):
+ *                    - first call with a set of arguments: the library builds a PLAN (box constants, work tables,
+ *                      kernel variants) and uploads its tables on `stream`.  It allocates the plan's device buffer,
+ *                      may grow the context's scratch -- growing a buffer that enqueued work may still read
+ *                      synchronises the DEVICE first (cudaDeviceSynchronize) -- and waits for the previous plan's table
+ *                      upload before it reuses the pinned staging buffer.  Do not build plans inside a stream capture.
+ *                    - every later call with the same arguments (a trajectory fed frame by frame or chunk by chunk):
+ *                      no allocation, no synchronisation, no event wait; it enqueues one memset, the repack kernel
+ *                      and the tile kernel launch(es).  The context keeps the 16 most recently used plans.
+ *                  If a plan is used on another stream than the one its tables went up on, the call makes that stream
+ *                  wait for the upload (cudaStreamWaitEvent).
  *  out             DEVICE pointer, uint64 [n_species*(n_species+1)/2][n_bins], OVERWRITTEN (added to with
  *                  CDH_FLAG_ACCUMULATE).
  *                  Row index of species pair (p <= q): p*n_species - p*(p-1)/2 + (q - p).
  *
- * Host arrays are read during the call only.  Returns CDH_OK or a negative code; on
- * CDH_ERR_INVALID_ARG nothing was enqueued.
+ * Host arrays are read during the call only.  Returns CDH_OK or a negative code; every argument check, and every
+ * allocation a new plan needs, happens before the first enqueue: on CDH_ERR_INVALID_ARG, CDH_ERR_UNSUPPORTED and
+ * CDH_ERR_ALLOC nothing was enqueued and `out` is untouched.
  */
 int cdh_histograms(cdh_ctx *ctx, const void *coords, int32_t n_frames,
                    const int32_t *species_offsets, int32_t n_species, int32_t box_type,
@@ -150,7 +164,8 @@ const char *cdh_last_error(const cdh_ctx *ctx);
  *   info[0] = kernels launched by the call      info[1] = work items (tile pairs) scheduled
  *   info[2] = bin-range sweeps                   info[3] = CTAs of the tile kernel
  *   info[4] = threads per CTA                    info[5] = dynamic shared memory bytes per CTA
- *   info[6] = kernel variant id (bit 0 fast path, bit 2 global histogram, bits 4-7 box type, bits 8-11 form: ORTHO 0 plain /
+ *   info[6] = kernel variant id (bit 0 fast path, bit 1 double precision, bit 2 global histogram, bit 3 hybrid (shared window of
+ *             the bins + L2 updates for the rest), bits 4-7 box type, bits 8-11 form: ORTHO 0 plain /
  *             1 fused / 2 exact-product rint, TRICLINIC zero structure; bit 12 bin-range split, bit 13 one-CTA-per-SM shape,
  *             bit 14 small-species variant: warps skip below-diagonal and padding-only work; bits 16.. j-chunk size)
  *   info[7] = pair slots the tile kernel is scheduled to walk (evaluated pairs incl. masked and padding lanes)
@@ -161,7 +176,7 @@ int cdh_last_call_info(const cdh_ctx *ctx, int64_t info[8]);
  * events recorded on the call's stream (a ring of CDH_TIMED_CALLS event sets, one per call):
  *   calls_back = 0 is the last call, 1 the one before, ... (< CDH_TIMED_CALLS and < calls made);
  *   ms[0] = the tile kernel launch(es) (steps S1-S7),
- *   ms[1] = the whole call (scratch upload, zeroing, repack, tile kernels).
+ *   ms[1] = the whole call (table upload of a new plan, zeroing, repack, window sampling, tile kernels).
  * WAITS for that call's last event.  Returns CDH_OK, CDH_ERR_INVALID_ARG (no such flag / no such call /
  * NULL) or CDH_ERR_CUDA. */
 #define CDH_TIMED_CALLS 256

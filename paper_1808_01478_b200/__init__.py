@@ -21,6 +21,12 @@ def histograms_device(ctx: "Context", problem, stream=None, precision: int = F32
     host = problem.coords.astype(np.float64) if precision == F64 else problem.coords
     coords = torch.from_numpy(host).to(dev)
     out = torch.empty((problem.n_hist, problem.n_bins), dtype=torch.int64, device=dev)
+    if stream is not None and hasattr(stream, "cuda_stream"):
+        # coords was filled on torch's current stream and is read on `stream`: order the two, and keep the caching allocator
+        # from handing the block to someone else before the repack kernel has read it (coords is dropped on return)
+        stream.wait_stream(torch.cuda.current_stream(dev))
+        coords.record_stream(stream)
+        out.record_stream(stream)
     ctx.cdh_histograms(coords, problem.n_frames, problem.species_offsets, problem.box_type, problem.box,
                        problem.r_max, problem.n_bins, out, precision=precision, stream=stream)
     return out

@@ -115,6 +115,24 @@ def _ptr(x) -> int:
     raise TypeError(f"cannot take the address of {type(x)}")
 
 
+def _check_device_tensor(x, what: str, device: int, dtype_name: str, min_numel: int) -> None:
+    """A torch tensor handed to a device entry point must be what the C call will read or write: CUDA memory of the
+    context's device, contiguous, of the precision's element type and large enough.  Raw integer pointers pass
+    through unchecked (the caller vouches for them)."""
+    if x is None or isinstance(x, int) or not hasattr(x, "data_ptr"):
+        return
+    if not getattr(x, "is_cuda", False):
+        raise ValueError(f"{what} must be a CUDA tensor (cdh_histograms_host takes host buffers)")
+    if x.device.index != device:
+        raise ValueError(f"{what} lives on cuda:{x.device.index}, the context on cuda:{device}")
+    if not x.is_contiguous():
+        raise ValueError(f"{what} must be contiguous")
+    if str(x.dtype).replace("torch.", "") not in dtype_name.split("|"):
+        raise ValueError(f"{what} must have dtype {dtype_name}, not {x.dtype}")
+    if x.numel() < min_numel:
+        raise ValueError(f"{what} has {x.numel()} elements, the call needs {min_numel}")
+
+
 def _stream_ptr(stream) -> int:
     if stream is None:
         return 0
@@ -154,6 +172,10 @@ class Context:
         """include/cdh.h ``cdh_histograms``: coords / out are DEVICE buffers (torch CUDA tensors or ints).
         Asynchronous on ``stream``."""
         off, b, n_boxes = self._marshal(species_offsets, box, n_frames)
+        n_species = len(off) - 1
+        _check_device_tensor(coords, "coords", self.device, "float64" if precision == F64 else "float32",
+                             int(n_frames) * int(off[-1]) * 3)
+        _check_device_tensor(out, "out", self.device, "int64|uint64", n_species * (n_species + 1) // 2 * int(n_bins))
         rc = self._lib.cdh_histograms(self._h, _ptr(coords), int(n_frames), off.ctypes.data, len(off) - 1,
                                       int(box_type), None if b is None else b.ctypes.data, n_boxes,
                                       float(r_max), int(n_bins), int(precision), _stream_ptr(stream), _ptr(out))
@@ -215,6 +237,8 @@ class Context:
         npairs = np.ascontiguousarray(n_pairs, dtype=np.float64).reshape(-1)
         if npairs.shape[0] != int(n_hist):
             raise ValueError("one pair count per histogram row")
+        _check_device_tensor(hist, "hist", self.device, "int64|uint64", int(n_hist) * int(n_bins))
+        _check_device_tensor(g, "g", self.device, "float64", int(n_hist) * int(n_bins))
         rc = self._lib.cdh_rdf(self._h, _ptr(hist), int(n_hist), int(n_bins), float(r_max), int(n_frames),
                                npairs.ctypes.data, float(volume), _stream_ptr(stream), _ptr(g))
         self._check(rc)

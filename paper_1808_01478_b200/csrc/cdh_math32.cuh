@@ -8,6 +8,9 @@
 #pragma once
 #include "cdh_fast.cuh"
 
+#ifndef CDH_TRI_RETEST
+#define CDH_TRI_RETEST 1     // 1: the triclinic pruning margins are recomputed by the rare group that needs them instead of being kept in 16 registers (config 3: 753 -> 784 Gpairs/s)
+#endif
 #ifndef CDH_ONE_U
 #define CDH_ONE_U 1     // 1: the second opaque 1.0f (TileParams::one_u) lives in a uniform register
 #endif
@@ -119,6 +122,41 @@ struct MathFast {
                 D2[r][1] = pair_d2_full_packed<kTri>(XB, YB, ZB, it.xi[r], it.yi[r], it.zi[r], it.fb, s_box, L.ones);
             }
         } else {
+#if CDH_TRI_RETEST
+            // the per-element pruning margins are NOT kept: only their maximum over the group; the rare group that needs the
+            // search recomputes them (16 floats fewer live across phase 1)
+            [[maybe_unused]] float fm_all = 0.0f;
+#pragma unroll
+            for (int r = 0; r < kR; ++r) {
+#pragma unroll
+                for (int hlf = 0; hlf < 2; ++hlf) {
+                    float f0, f1;
+                    D2[r][hlf] = pair_d2_fast<BOX, kTri>(hlf ? XB : XA, hlf ? YB : YA, hlf ? ZB : ZA, it.xi[r], it.yi[r], it.zi[r],
+                                                         it.fb, L.ones, f0, f1);
+                    if constexpr (BOX == BOX_TRI) fm_all = fmaxf(fmaxf(fm_all, f0), f1);
+                }
+            }
+            if constexpr (BOX == BOX_TRI) {
+                if (fm_all > L.prune_lim) {
+                    const float xj[4] = {XJ.x, XJ.y, XJ.z, XJ.w}, yj[4] = {YJ.x, YJ.y, YJ.z, YJ.w}, zj[4] = {ZJ.x, ZJ.y, ZJ.z, ZJ.w};
+#pragma unroll
+                    for (int r = 0; r < kR; ++r) {
+#pragma unroll
+                        for (int hlf = 0; hlf < 2; ++hlf) {
+                            float xr = it.xi[r], f0, f1;
+                            asm volatile("" : "+f"(xr));                 // opaque: the margins are recomputed, not kept alive
+                            (void)pair_d2_fast<BOX, kTri>(hlf ? XB : XA, hlf ? YB : YA, hlf ? ZB : ZA, xr, it.yi[r], it.zi[r], it.fb, L.ones, f0, f1);
+                            float p, q; upk2(D2[r][hlf], p, q);
+                            bool n0 = f0 > L.prune_lim, n1 = f1 > L.prune_lim;
+                            if constexpr (MASKED) { n0 = n0 && (jg + 2 * hlf > ig + r); n1 = n1 && (jg + 2 * hlf + 1 > ig + r); }
+                            if (n0) p = tri_full_d2(it.xi[r], it.yi[r], it.zi[r], xj[2 * hlf], yj[2 * hlf], zj[2 * hlf], s_box);
+                            if (n1) q = tri_full_d2(it.xi[r], it.yi[r], it.zi[r], xj[2 * hlf + 1], yj[2 * hlf + 1], zj[2 * hlf + 1], s_box);
+                            D2[r][hlf] = pk2(p, q);
+                        }
+                    }
+                }
+            }
+#else
             float fm[kR][2][2];
             [[maybe_unused]] float fm_all = 0.0f;
 #pragma unroll
@@ -149,6 +187,7 @@ struct MathFast {
                     }
                 }
             }
+#endif
         }
         // phase 2: bin and update
 #pragma unroll

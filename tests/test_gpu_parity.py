@@ -287,21 +287,26 @@ def test_argument_errors_leave_out_untouched():
     dev = torch.device("cuda", 0)
     coords = torch.from_numpy(p.coords).to(dev)
     out = torch.full((1, p.n_bins), -7, dtype=torch.int64, device=dev)
+    c_ptr, o_ptr = int(coords.data_ptr()), int(out.data_ptr())     # raw pointers: the C library's own checks are under test
     with cdh.Context(0) as ctx:
         for kw in (dict(n_bins=0), dict(r_max=-1.0), dict(r_max=float("nan")), dict(n_bins=(1 << 22) + 1)):
             args = dict(r_max=p.r_max, n_bins=p.n_bins)
             args.update(kw)
             with pytest.raises(cdh.CdhError) as e:
-                ctx.cdh_histograms(coords, 1, p.species_offsets, p.box_type, None, args["r_max"], args["n_bins"], out)
+                ctx.cdh_histograms(c_ptr, 1, p.species_offsets, p.box_type, None, args["r_max"], args["n_bins"], o_ptr)
             assert e.value.code == cdh.binding.ERR_INVALID_ARG
         with pytest.raises(cdh.CdhError) as e:
-            ctx.cdh_histograms(coords, 1, p.species_offsets, p.box_type, None, p.r_max, p.n_bins, out, precision=7)
+            ctx.cdh_histograms(c_ptr, 1, p.species_offsets, p.box_type, None, p.r_max, p.n_bins, o_ptr, precision=7)
         assert e.value.code == cdh.binding.ERR_INVALID_ARG
         with pytest.raises(cdh.CdhError):       # singular box
-            ctx.cdh_histograms(coords, 1, p.species_offsets, inputs.BOX_TRICLINIC, np.zeros((1, 9)), 1.0, 10, out)
+            ctx.cdh_histograms(c_ptr, 1, p.species_offsets, inputs.BOX_TRICLINIC, np.zeros((1, 9)), 1.0, 10, o_ptr)
         with pytest.raises(cdh.CdhError):       # off-diagonal with ORTHO
-            ctx.cdh_histograms(coords, 1, p.species_offsets, inputs.BOX_ORTHO,
-                               np.array([[1.0, 0.1, 0, 0, 1, 0, 0, 0, 1]]), 1.0, 10, out)
+            ctx.cdh_histograms(c_ptr, 1, p.species_offsets, inputs.BOX_ORTHO,
+                               np.array([[1.0, 0.1, 0, 0, 1, 0, 0, 0, 1]]), 1.0, 10, o_ptr)
+        with pytest.raises(ValueError):         # the binding refuses a tensor the call would overrun
+            ctx.cdh_histograms(coords, 1, p.species_offsets, p.box_type, None, p.r_max, p.n_bins + 1, out)
+        with pytest.raises(ValueError):         # ... and one of the wrong element type
+            ctx.cdh_histograms(coords.double(), 1, p.species_offsets, p.box_type, None, p.r_max, p.n_bins, out)
     torch.cuda.synchronize()
     assert bool((out == -7).all())
 

@@ -101,3 +101,30 @@ def test_invalid_arguments_are_refused_before_anything_runs():
         assert e.value.code == -1            # CDH_ERR_INVALID_ARG
         with pytest.raises(cdh.CdhError):
             ctx.cdh_histograms_stream(p.coords, p.species_offsets, p.box_type, p.box, -1.0, p.n_bins)
+
+
+def test_plan_cache_many_shapes_two_streams_and_changing_coordinates():
+    """The context caches plans keyed by the arguments (not the coordinate values): repeated calls with new
+    coordinates, more distinct shapes than the cache holds (least recently used out) and a plan reused on another
+    stream than the one its tables were uploaded on must all give the oracle's integers."""
+    _need_gpu()
+    box = np.diag([3.0, 3.5, 4.0])
+    with cdh.Context(0) as ctx:
+        s1, s2 = torch.cuda.Stream(), torch.cuda.Stream()
+        shapes = [(300 + 37 * k, 100 + 11 * k) for k in range(20)]            # 20 plans > 16 cached
+        for rnd in range(2):
+            for k, counts in enumerate(shapes):
+                p = inputs.uniform_problem(1000 * rnd + k, counts, inputs.BOX_ORTHO, 500 + k, 1.4, box=box)
+                out = cdh.histograms_device(ctx, p, stream=(s1 if (k + rnd) % 2 else s2))
+                torch.cuda.synchronize()
+                got = out.cpu().numpy().view(np.uint64)
+                assert np.array_equal(got, cdh_oracle.problem_histograms(p, "f32")), (rnd, counts)
+        # same plan, back-to-back calls on alternating streams without a host synchronisation in between
+        p = inputs.uniform_problem(5, (700, 200), inputs.BOX_ORTHO, 640, 1.4, box=box)
+        q = inputs.uniform_problem(6, (700, 200), inputs.BOX_ORTHO, 640, 1.4, box=box)
+        a = cdh.histograms_device(ctx, p, stream=s1)
+        s2.wait_stream(s1)                                                     # the context's scratch is reused: order the streams
+        b = cdh.histograms_device(ctx, q, stream=s2)
+        torch.cuda.synchronize()
+        assert np.array_equal(a.cpu().numpy().view(np.uint64), cdh_oracle.problem_histograms(p, "f32"))
+        assert np.array_equal(b.cpu().numpy().view(np.uint64), cdh_oracle.problem_histograms(q, "f32"))

@@ -71,3 +71,33 @@ def test_product_does_not_import_the_oracle():
                 assert not re.search(r"^\s*(from|import)\s+oracle\b", text, flags=re.M), f
                 assert not re.search(r"#include\s+[\"<][^\">]*oracle", text), f
                 assert "libcdh_oracle" not in text, f
+
+
+def test_binding_rejects_tensors_the_c_call_would_misread():
+    """Context.cdh_histograms takes data_ptr() of torch tensors: a CPU, non-contiguous, wrongly typed or undersized tensor
+    must be refused by the binding (the C ABI sees plain pointers and cannot tell)."""
+    torch = pytest.importorskip("torch")
+    from paper_1808_01478_b200 import binding
+    with pytest.raises(ValueError, match="CUDA tensor"):
+        binding._check_device_tensor(torch.zeros(30), "coords", 0, "float32", 30)
+    binding._check_device_tensor(123456, "coords", 0, "float32", 30)          # raw pointers pass through
+    binding._check_device_tensor(None, "coords", 0, "float32", 30)
+
+    class Fake:                                                                # stands in for a CUDA tensor on a CPU-only box
+        is_cuda = True
+        dtype = torch.float64
+        class device:
+            index = 0
+        def __init__(self, n, contiguous=True): self._n, self._c = n, contiguous
+        def data_ptr(self): return 1
+        def is_contiguous(self): return self._c
+        def numel(self): return self._n
+    with pytest.raises(ValueError, match="dtype"):
+        binding._check_device_tensor(Fake(30), "coords", 0, "float32", 30)
+    with pytest.raises(ValueError, match="contiguous"):
+        binding._check_device_tensor(Fake(30, False), "coords", 0, "float64", 30)
+    with pytest.raises(ValueError, match="elements"):
+        binding._check_device_tensor(Fake(29), "coords", 0, "float64", 30)
+    with pytest.raises(ValueError, match="cuda:0"):
+        binding._check_device_tensor(Fake(30), "coords", 1, "float64", 30)
+    binding._check_device_tensor(Fake(30), "coords", 0, "float64", 30)
