@@ -30,7 +30,7 @@ FLAG_MAX_SMEM_BINS_SHIFT = 8
 
 EXPORTS = ["cdh_create", "cdh_histograms", "cdh_histograms_host", "cdh_histograms_stream", "cdh_destroy", "cdh_strerror",
            "cdh_last_error", "cdh_last_call_info", "cdh_call_kernel_ms", "cdh_rdf",
-           "cdh_bench_fp32_rate", "cdh_bench_shared_atomics", "cdh_bench_inner_loop", "cdh_selftest_sqrt", "cdh_selftest_sqrt_f64",
+           "cdh_bench_fp32_rate", "cdh_bench_shared_atomics", "cdh_bench_inner_loop", "cdh_bench_dsmem_atomics", "cdh_selftest_sqrt", "cdh_selftest_sqrt_f64",
            "cdh_host_d2_threshold_bits", "cdh_host_fused_rint_constant", "cdh_host_work_items"]
 
 
@@ -81,6 +81,8 @@ def load(path: Optional[str] = None) -> ctypes.CDLL:
     lib.cdh_bench_shared_atomics.argtypes = [ctypes.c_int, ctypes.c_int, ctypes.c_int, vp, ctypes.c_int, dbl,
                                              ctypes.c_int, ctypes.c_int, ctypes.c_int, vp,
                                              ctypes.POINTER(dbl), ctypes.POINTER(dbl), ctypes.POINTER(dbl)]
+    lib.cdh_bench_dsmem_atomics.restype = ctypes.c_int
+    lib.cdh_bench_dsmem_atomics.argtypes = [ctypes.c_int, ctypes.c_int, ctypes.c_int, vp, ctypes.POINTER(dbl), ctypes.POINTER(dbl)]
     lib.cdh_bench_inner_loop.restype = ctypes.c_int
     lib.cdh_bench_inner_loop.argtypes = [ctypes.c_int, ctypes.c_int, ctypes.c_int, ctypes.c_int, vp, ctypes.POINTER(dbl), ctypes.POINTER(dbl)]
     lib.cdh_selftest_sqrt.restype = ctypes.c_int
@@ -302,6 +304,16 @@ def cdh_bench_shared_atomics(pattern: int, op: int, n_bins: int, samples=None, n
     if rc != OK:
         raise CdhError(rc, cdh_strerror(rc))
     return r.value, ms.value, ms0.value
+
+
+def cdh_bench_dsmem_atomics(cluster_size: int, bins_per_cta: int = 25000, iters: int = 512, stream=None):
+    """include/cdh_bench.h ``cdh_bench_dsmem_atomics``: (updates per second, kernel ms) of cluster-distributed shared atomics."""
+    lib = load()
+    r, ms = ctypes.c_double(), ctypes.c_double()
+    rc = lib.cdh_bench_dsmem_atomics(int(cluster_size), int(bins_per_cta), int(iters), _stream_ptr(stream), ctypes.byref(r), ctypes.byref(ms))
+    if rc != OK:
+        raise CdhError(rc, cdh_strerror(rc))
+    return r.value, ms.value
 
 
 def cdh_bench_inner_loop(box: int, level: int, free_alu: int = 0, iters: int = 40, stream=None):
