@@ -462,3 +462,55 @@ def test_small_species_take_the_skip_variants(box_type):
     got, info = gpu_hist(big)
     assert not info["skip"], info
     assert_same(got, oracle_hist(big), f"large species, box_type {box_type}")
+
+
+def test_no_box_clean_form_and_everything_that_must_switch_it_off():
+    """No box: when every distance of the call is provably below r_max and no coordinate is NaN the kernel leaves out the
+    threshold compare (KIND_CLEAN, cdh_sched.cuh).  The device decides from the coordinate extent the repack kernel
+    measures; each of these inputs must give the oracle's integers whichever form runs."""
+    g = np.random.Generator(np.random.PCG64(77))
+    n = 9000                                                    # several i-tiles and a ragged tail
+    base = g.random((n, 3)).astype(np.float32)
+    cases = {"clean": (base, math.sqrt(3.0))}
+    x = base.copy(); x[4321] = x[17]; x[8999] = x[17]           # coincident particles: d2 = 0 inside the clean form
+    cases["coincident"] = (x, math.sqrt(3.0))
+    x = base.copy(); x[5000, 1] = np.nan                        # a NaN coordinate: its pairs are dropped, the form is general
+    cases["nan"] = (x, math.sqrt(3.0))
+    x = base.copy(); x[123, 0] = np.inf
+    cases["inf"] = (x, math.sqrt(3.0))
+    cases["r_max inside the extent"] = (base, 1.2)              # some pairs are beyond r_max
+    x = base.copy(); x[0] = (0.0, 0.0, 0.0); x[1] = (1.0, 1.0, 1.0)
+    cases["corner to corner"] = (x, math.sqrt(3.0))             # d = fl(sqrt(3)) is NOT below (float)r_max: dropped
+    for name, (pts, r_max) in cases.items():
+        for offsets in ([0, n], [0, 4097, n]):
+            p = inputs.Problem(name, np.ascontiguousarray(pts[None]), np.array(offsets, dtype=np.int32), inputs.BOX_NONE, None,
+                               r_max, 3000)
+            got, info = gpu_hist(p)
+            assert_same(got, oracle_hist(p), f"{name}, offsets {offsets}: {info}")
+    p = inputs.Problem("clean", np.ascontiguousarray(base[None]), np.array([0, n], dtype=np.int32), inputs.BOX_NONE, None,
+                       math.sqrt(3.0), 3000)
+    assert int(gpu_hist(p)[0].sum()) == n * (n - 1) // 2
+
+
+def test_hybrid_window_with_frames_accumulate_and_per_frame_boxes():
+    """MODE_HYBRID next to the other features: several frames with their own boxes, CDH_FLAG_ACCUMULATE (the result is
+    not zeroed), and a bin count one above what the shared memory holds."""
+    _need_gpu()
+    f, counts = 3, (1500, 700)
+    g = np.random.Generator(np.random.PCG64(5))
+    boxes = np.stack([np.diag([4.0 + 0.1 * k, 4.5, 5.0 - 0.1 * k]) for k in range(f)]).reshape(f, 9)
+    coords = (g.random((f, sum(counts), 3)) * 5.0).astype(np.float32)
+    for n_bins in (56_403, 90_000):
+        p = inputs.Problem("hyb_frames", coords, np.array([0, 1500, 2200], dtype=np.int32), inputs.BOX_ORTHO, boxes, 2.0, n_bins)
+        want = oracle_hist(p)
+        got, info = gpu_hist(p)
+        assert info["hybrid"], info
+        assert_same(got, want, f"{n_bins} bins, per-frame boxes: {info}")
+        with cdh.Context(0, cdh.FLAG_ACCUMULATE) as ctx:
+            dev = torch.device("cuda", 0)
+            out = torch.zeros((p.n_hist, n_bins), dtype=torch.int64, device=dev)
+            for k in range(f):                                   # frame by frame into the same result
+                c = torch.from_numpy(np.ascontiguousarray(coords[k:k + 1])).to(dev)
+                ctx.cdh_histograms(c, 1, p.species_offsets, p.box_type, boxes[k:k + 1], p.r_max, n_bins, out)
+            torch.cuda.synchronize()
+            assert_same(out.cpu().numpy().view(np.uint64), want, f"{n_bins} bins, accumulated frame by frame")
