@@ -250,7 +250,7 @@ class Context:
         self._check(self._lib.cdh_last_call_info(self._h, arr))
         v = list(arr)
         return {"launches": v[0], "items": v[1], "sweeps": v[2], "ctas": v[3], "threads": v[4],
-                "smem_bytes": v[5], "variant": v[6], "tj": v[6] >> 16, "fast": bool(v[6] & 1), "global_hist": bool(v[6] & 4), "hybrid": bool(v[6] & 8), "form": (v[6] >> 8) & 15, "skip": bool(v[6] & (1 << 14)),
+                "smem_bytes": v[5], "variant": v[6], "tj": v[6] >> 16, "fast": bool(v[6] & 1), "global_hist": bool(v[6] & 4), "hybrid": bool(v[6] & 8), "form": (v[6] >> 8) & 15, "skip": bool(v[6] & (1 << 14)), "full_range": bool(v[6] & (1 << 15)),
                 "padded_pairs": v[7]}
 
     def call_kernel_ms(self, calls_back: int = 0):

@@ -35,7 +35,7 @@ struct Plan {
     size_t o_rows = 0, o_boxes = 0, o_off = 0, o_pad = 0, o_rowseg = 0, o_win = 0;
     std::vector<Launch> launches;
     int smem_bytes = 0, mode = MODE_SHARED;
-    uint32_t grid = 0, n_items = 0, n_rows = 0, tj = 0, smem_bins = 0, n_stages = 2;
+    uint32_t grid = 0, n_items = 0, n_rows = 0, tj = 0, smem_bins = 0, n_stages = 2, keep_bins = 0;
     double r_max = 0.0;
     float rmax_f = 0.f, scale_f = 0.f;
     uint32_t thr2_bits = 0;
@@ -364,6 +364,31 @@ int build_plan(cdh_ctx* ctx, cudaStream_t stream, int32_t n_frames, const int32_
         } else if ((uint64_t)n_bins > (uint64_t)CDH_HYBRID_MAX_RATIO * cap_two) { mode = MODE_GLOBAL; smem_bins = 0; }
         else { mode = MODE_HYBRID; smem_bins = cap_two; }
     }
+    // Orthorhombic box, whole histogram in shared memory: give the private histogram a slot for EVERY reachable distance
+    // (wrapped components are within L/2, so d <= |diagonal|/2) and flush only the first n_bins of them.  Stages without
+    // padding then need no threshold compare and no trash select (CLEAN form, cdh_fast.cuh).  Exact iff no dropped pair can
+    // share a slot with a kept one: bin(thr2) >= n_bins, and no kept pair rounds up into slot n_bins (reading Q3).
+    uint32_t keep_bins = 0;
+#ifndef CDH_ORTHO_CLEAN
+#define CDH_ORTHO_CLEAN 1
+#endif
+    if (CDH_ORTHO_CLEAN && !f64 && box_type == CDH_BOX_ORTHO && mode == MODE_SHARED && !use_simple_only && !(ctx->flags & CDH_FLAG_NO_PRUNE)) {
+        const float thr2 = bits_f32(d2_threshold_bits(rmax_f));
+        const float b_thr = floorf(sqrtf(thr2) * scale_f), b_prev = floorf(sqrtf(std::nextafterf(thr2, 0.0f)) * scale_f);
+        double d2max = 0.0;
+        for (int b = 0; b < nb; ++b) {
+            double acc = 0.0;
+            for (int c = 0; c < 3; ++c) { const double h = std::fabs((double)boxes32[b].L[c]) * (0.5 + std::ldexp(1.0, -18)); acc += h * h; }
+            d2max = std::fmax(d2max, acc);
+        }
+        const double slots = std::floor(std::sqrt(d2max) * (double)scale_f * (1.0 + 1e-6)) + 3.0;
+        if (b_thr >= (float)n_bins && b_prev <= (float)(n_bins - 1) && slots < 4.0e6 && slots > (double)n_bins) {
+            const uint32_t all = (uint32_t)slots;
+            // measured: config 4 (3 resident CTAs either way) 1,258 -> 1,356 Gpairs/s; config 2 (2 instead of 3 resident CTAs)
+            // 1,231 -> 1,308: the two instructions saved per pair outweigh the lost CTA, so the form is taken whenever it fits
+            if (all <= cap_two) { keep_bins = (uint32_t)n_bins; smem_bins = all; }
+        }
+    }
     if (mode != MODE_GLOBAL && smem_bins > cap_ring) n_stages = 2;
     const int smem_bytes = smem_fixed(precision, (int)n_stages) + 4 * ((int)smem_bins + 2);
     const bool big = 2 * (smem_bytes + 1024) > 228 * 1024 || mode == MODE_HYBRID;          // one CTA per SM
@@ -471,14 +496,14 @@ int build_plan(cdh_ctx* ctx, cudaStream_t stream, int32_t n_frames, const int32_
     pl->repack_blocks = blocks_per_frame * (uint32_t)n_frames;
     pl->smem_bytes = smem_bytes; pl->mode = mode; pl->n_items = (uint32_t)wt.n_items; pl->n_rows = (uint32_t)wt.rows.size() - 1;
     pl->grid = grid_full < pl->n_items ? grid_full : pl->n_items;
-    pl->tj = tj; pl->smem_bins = smem_bins; pl->n_stages = n_stages;
+    pl->tj = tj; pl->smem_bins = smem_bins; pl->n_stages = n_stages; pl->keep_bins = keep_bins;
     pl->r_max = r_max; pl->rmax_f = rmax_f; pl->scale_f = scale_f; pl->thr2_bits = f64 ? 0u : d2_threshold_bits(rmax_f);
     if (f64) pl->box0_64 = boxes64[0];
     const int n_launch = (frame_slots > 0 ? 1 : 0) + (wt.n_items > 0 ? (int)pl->launches.size() + (mode == MODE_HYBRID ? 1 : 0) : 0);
     pl->info[0] = n_launch; pl->info[1] = (int64_t)wt.n_items; pl->info[2] = sp.n_sweeps; pl->info[3] = pl->grid;
     pl->info[4] = vf.threads; pl->info[5] = smem_bytes;
     pl->info[6] = (f64 ? 2 : (use_simple_only ? 0 : 1)) | ((int)(mode == MODE_GLOBAL) << 2) | ((int)(mode == MODE_HYBRID) << 3) | (box_type << 4) |
-                  ((form & 15) << 8) | ((int)(mode == MODE_SPLIT) << 12) | ((int)big << 13) | ((int)skip << 14) | ((int64_t)tj << 16);
+                  ((form & 15) << 8) | ((int)(mode == MODE_SPLIT) << 12) | ((int)big << 13) | ((int)skip << 14) | ((int)(keep_bins != 0) << 15) | ((int64_t)tj << 16);
     pl->info[7] = (int64_t)wt.padded_pairs;
 
     // least recently used plan out (its tables may still be read by enqueued work: wait for the device first)
@@ -572,7 +597,7 @@ int enqueue_plan(cdh_ctx* ctx, const Plan& pl, const void* coords, cudaStream_t 
         }
         for (size_t k = 0; k < pl.launches.size(); ++k) {
             c.counter = ctx->d_scalars + k;
-            if (!f64) { tp.range_lo = pl.launches[k].lo; tp.range_hi = pl.launches[k].hi; }
+            if (!f64) { tp.range_lo = pl.launches[k].lo; tp.range_hi = pl.launches[k].hi; tp.keep_bins = k == 0 ? pl.keep_bins : 0u; }
             void* args[1] = {f64 ? (void*)&tp64 : (void*)&tp};
             CDH_CUDA(cudaLaunchKernel(pl.launches[k].v.fn, dim3(pl.grid), dim3((unsigned)pl.launches[k].v.threads), args,
                                       (size_t)pl.smem_bytes, stream));

@@ -90,6 +90,9 @@ struct TileParams : TileCommon {
                                 // in a uniform register (the first one must be a vector register where the addend is an immediate)
     float range_lo, range_hi;   // periodic boxes: this launch does the work iff range_lo < frac_range() <= range_hi
                                 // (range_hi = +inf: no upper limit, and a NaN range counts as above range_lo)
+    uint32_t keep_bins;         // 0, or (orthorhombic box, this launch only) the number of flushed slots of a private histogram that
+                                // has a slot for EVERY reachable distance: stages without padding then need no threshold compare
+                                // (DESIGN.md "CLEAN form"); smem_bins is the full slot count
 };
 
 // ---------------------------------------------------------------------------------------------

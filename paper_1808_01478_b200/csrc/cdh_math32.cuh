@@ -41,7 +41,7 @@ struct MathFast {
     using Params = TileParams;
     static constexpr int kStageBytes = cdh::kStageBytes;
     static constexpr bool kPeriodic = BOX != BOX_NONE;
-    static constexpr bool kHasClean = BOX == BOX_NONE;
+    static constexpr bool kHasClean = BOX == BOX_NONE || BOX == BOX_ORTHO;
     static constexpr int kUnroll = 1;
     static constexpr bool kNoPrune = BOX == BOX_TRI && (TRI & TRI_NOPRUNE) != 0;
     static constexpr int kTri = TRI & ~TRI_NOPRUNE;
@@ -70,6 +70,9 @@ struct MathFast {
             if (!mine) return false;
             // TRI_WIDE: the error of s_k grows linearly with the range, and so must the margin (2x the 2^-17 of range 1.49)
             if constexpr (BOX == BOX_TRI && (TRI & TRI_WIDE) != 0) L.prune_lim = 0.5f - kPruneDelta * 2.0f * fmaxf(1.0f, range * (1.0f / 1.49f));
+            // orthorhombic, fractional range <= 1.49: every wrapped component is within L/2 (1 + 2^-18), so the host could size
+            // the private histogram for every reachable distance (keep_bins != 0); no NaN coordinate in the call
+            if constexpr (BOX == BOX_ORTHO) L.clean = P.keep_bins != 0u && __ldg(P.range_keys + 6) == 0u;
         } else {
             L.clean = __float_as_uint(coord_extent2_ru(P.range_keys)) < P.thr2_bits;
         }
@@ -85,6 +88,7 @@ struct MathFast {
             hv.lim = min(P.smem_bins, P.n_bins - hv.lo);
         } else {
             hv.lo = seg.bin_lo; hv.lim = seg.bin_cnt + seg.last_sweep;
+            if constexpr (BOX == BOX_ORTHO && MODE == MODE_SHARED) if (P.keep_bins != 0u) hv.lim = P.keep_bins;   // slots beyond: dropped pairs
         }
     }
 

@@ -514,3 +514,37 @@ def test_hybrid_window_with_frames_accumulate_and_per_frame_boxes():
                 ctx.cdh_histograms(c, 1, p.species_offsets, p.box_type, boxes[k:k + 1], p.r_max, n_bins, out)
             torch.cuda.synchronize()
             assert_same(out.cpu().numpy().view(np.uint64), want, f"{n_bins} bins, accumulated frame by frame")
+
+
+def test_orthorhombic_full_range_private_histogram():
+    """Orthorhombic box: when no dropped pair can share a bin slot with a kept one (the host checks bin(thr2) >= n_bins and
+    that no kept pair rounds up into slot n_bins) the private histogram gets a slot for every reachable distance and stages
+    without padding skip the threshold compare (info["full_range"]).  Taken or not, the integers are the oracle's."""
+    _need_gpu()
+    cases = [
+        # (box diag, r_max, n_bins, counts): dyadic scale -> the form is taken
+        ((10.0, 10.0, 10.0), 5.0, 10000, (3000, 5200)),
+        ((8.0, 9.0, 7.5), 3.75, 3000, (4100, 1000)),           # anisotropic box, r_max = half the shortest edge
+        ((6.0, 6.0, 6.0), 1.0, 512, (5000,)),                  # few pairs kept: most updates land beyond n_bins
+        ((6.0, 6.0, 6.0), 5.0, 2048, (5000,)),                 # r_max beyond half the box: nearly every pair is kept
+        # scales that are not exact in fp32: taken or not depending on the rounding, exact either way
+        ((7.3, 8.1, 9.7), 3.65, 7777, (2500, 2600)),
+        ((5.123, 5.123, 5.123), 2.5615, 9999, (4097,)),
+        ((11.0, 11.0, 11.0), 5.5, 30011, (3000,)),             # the full-range histogram needs the one-CTA-per-SM shape
+    ]
+    taken = 0
+    for k, (diag, r_max, n_bins, counts) in enumerate(cases):
+        p = inputs.uniform_problem(500 + k, counts, inputs.BOX_ORTHO, n_bins, r_max, box=np.diag(diag), n_frames=2, spread=1.2)
+        got, info = gpu_hist(p)
+        taken += info["full_range"]
+        assert_same(got, oracle_hist(p), f"case {k} {diag} r_max {r_max} bins {n_bins}: {info}")
+        plain, info2 = gpu_hist(p, cdh.FLAG_NO_PRUNE)           # the pinned 5-operation form, no full-range histogram
+        assert not info2["full_range"]
+        assert_same(plain, got, f"case {k}: plain form")
+    assert taken >= 4
+    # a NaN coordinate switches the form off on the device (its pairs are dropped by the threshold compare)
+    p = inputs.uniform_problem(77, (3000, 1200), inputs.BOX_ORTHO, 4096, 4.0, box=np.diag((8.0, 8.0, 8.0)))
+    p.coords[0, 1234, 2] = np.nan
+    got, info = gpu_hist(p)
+    assert info["full_range"]
+    assert_same(got, oracle_hist(p), "NaN coordinate with the full-range histogram")
