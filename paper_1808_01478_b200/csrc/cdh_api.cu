@@ -372,17 +372,27 @@ int build_plan(cdh_ctx* ctx, cudaStream_t stream, int32_t n_frames, const int32_
 #ifndef CDH_ORTHO_CLEAN
 #define CDH_ORTHO_CLEAN 1
 #endif
-    if (CDH_ORTHO_CLEAN && !f64 && box_type == CDH_BOX_ORTHO && mode == MODE_SHARED && !use_simple_only && !(ctx->flags & CDH_FLAG_NO_PRUNE)) {
-        const float thr2 = bits_f32(d2_threshold_bits(rmax_f));
-        const float b_thr = floorf(sqrtf(thr2) * scale_f), b_prev = floorf(sqrtf(std::nextafterf(thr2, 0.0f)) * scale_f);
+    if (CDH_ORTHO_CLEAN && box_type == CDH_BOX_ORTHO && mode == MODE_SHARED && !use_simple_only && !(ctx->flags & CDH_FLAG_NO_PRUNE)) {
+        // the two bins that decide it, by the pinned operations of the precision: of the first dropped distance and of the last kept one
+        double b_thr, b_prev;
+        if (f64) {
+            const double scale_d = (double)n_bins / r_max;
+            b_thr = std::floor(r_max * scale_d); b_prev = std::floor(std::nextafter(r_max, 0.0) * scale_d);
+        } else {
+            const float thr2 = bits_f32(d2_threshold_bits(rmax_f));
+            b_thr = (double)floorf(sqrtf(thr2) * scale_f); b_prev = (double)floorf(sqrtf(std::nextafterf(thr2, 0.0f)) * scale_f);
+        }
         double d2max = 0.0;
         for (int b = 0; b < nb; ++b) {
             double acc = 0.0;
-            for (int c = 0; c < 3; ++c) { const double h = std::fabs((double)boxes32[b].L[c]) * (0.5 + std::ldexp(1.0, -18)); acc += h * h; }
+            for (int c = 0; c < 3; ++c) {
+                const double h = std::fabs(f64 ? boxes64[b].L[c] : (double)boxes32[b].L[c]) * (0.5 + std::ldexp(1.0, -18));
+                acc += h * h;
+            }
             d2max = std::fmax(d2max, acc);
         }
-        const double slots = std::floor(std::sqrt(d2max) * (double)scale_f * (1.0 + 1e-6)) + 3.0;
-        if (b_thr >= (float)n_bins && b_prev <= (float)(n_bins - 1) && slots < 4.0e6 && slots > (double)n_bins) {
+        const double slots = std::floor(std::sqrt(d2max) * (f64 ? (double)n_bins / r_max : (double)scale_f) * (1.0 + 1e-6)) + 3.0;
+        if (b_thr >= (double)n_bins && b_prev <= (double)(n_bins - 1) && slots < 4.0e6 && slots > (double)n_bins) {
             const uint32_t all = (uint32_t)slots;
             // measured: config 4 (3 resident CTAs either way) 1,258 -> 1,356 Gpairs/s; config 2 (2 instead of 3 resident CTAs)
             // 1,231 -> 1,308: the two instructions saved per pair outweigh the lost CTA, so the form is taken whenever it fits
@@ -574,7 +584,7 @@ int enqueue_plan(cdh_ctx* ctx, const Plan& pl, const void* coords, cudaStream_t 
         c.n_stages = pl.n_stages;
         if (f64) {
             tp64.pk = (const double*)ctx->d_pk; tp64.boxes = (const BoxConst64*)(d + pl.o_boxes);
-            tp64.rmax = pl.r_max; tp64.scale = (double)pl.n_bins / pl.r_max; tp64.box0 = pl.box0_64;
+            tp64.rmax = pl.r_max; tp64.scale = (double)pl.n_bins / pl.r_max; tp64.box0 = pl.box0_64; tp64.keep_bins = pl.keep_bins;
         } else {
             tp.pk = (const float*)ctx->d_pk; tp.boxes = (const BoxConst*)(d + pl.o_boxes);
             tp.rmax = pl.rmax_f; tp.scale = pl.scale_f; tp.thr2_bits = pl.thr2_bits; tp.one = 1.0f; tp.one_u = 1.0f;

@@ -28,6 +28,7 @@ struct TileParams64 : TileCommon {
     const double*   pk;
     const BoxConst64* boxes;
     double rmax, scale;         // r_max, n_bins / r_max
+    uint32_t keep_bins;         // orthorhombic full-range private histogram (as TileParams::keep_bins), else 0
     BoxConst64 box0;            // PBOX variants (one box for all frames): the constants sit in the kernel-parameter
                                 // constant bank and are used as c[0x0][..] operands, no shared-memory loads
 };
@@ -53,7 +54,7 @@ static __global__ void __launch_bounds__(256) repack_kernel_f64(const RepackPara
         for (uint64_t k = (uint64_t)blockIdx.x * 256u + threadIdx.x; k < P.zero_count; k += (uint64_t)gridDim.x * 256u) P.zero[k] = 0ull;
     const uint32_t f = blockIdx.x / P.blocks_per_frame;
     const uint32_t slot = (blockIdx.x % P.blocks_per_frame) * blockDim.x + threadIdx.x;
-    float fr[3] = {0.0f, 0.0f, 0.0f};
+    float fr[3] = {0.0f, 0.0f, 0.0f}, fr_lo[3] = {0.0f, 0.0f, 0.0f};     // upper / lower float bounds of the keyed quantity
     bool have = false;
     if (slot < P.frame_slots) {
         int lo = 0, hi = P.n_species;
@@ -70,21 +71,29 @@ static __global__ void __launch_bounds__(256) repack_kernel_f64(const RepackPara
             if (P.box_type == BOX_TRI) {      // only the triclinic pruning reads the range
                 const BoxConst64* bc = P.boxes + (P.n_boxes == 1 ? 0 : f);
 #pragma unroll
-                for (int q = 0; q < 3; ++q) fr[q] = (float)(bc->Binv[3 * q] * x + bc->Binv[3 * q + 1] * y + bc->Binv[3 * q + 2] * z);
+                for (int q = 0; q < 3; ++q) fr[q] = fr_lo[q] = (float)(bc->Binv[3 * q] * x + bc->Binv[3 * q + 1] * y + bc->Binv[3 * q + 2] * z);
                 have = (fr[0] == fr[0]) && (fr[1] == fr[1]) && (fr[2] == fr[2]);
+            } else if (P.box_type == BOX_ORTHO) {   // the full-range CLEAN form needs |x / L| < 2^20 (cdh_math: launch_begin)
+                const BoxConst64* bc = P.boxes + (P.n_boxes == 1 ? 0 : f);
+                fr[0] = fr_lo[0] = (float)(x * bc->invL[0]); fr[1] = fr_lo[1] = (float)(y * bc->invL[1]); fr[2] = fr_lo[2] = (float)(z * bc->invL[2]);
+                have = (fr[0] == fr[0]) && (fr[1] == fr[1]) && (fr[2] == fr[2]);
+            } else {                                // no box: float bounds of the coordinates, rounded OUTWARD
+                fr[0] = __double2float_ru(x); fr[1] = __double2float_ru(y); fr[2] = __double2float_ru(z);
+                fr_lo[0] = __double2float_rd(x); fr_lo[1] = __double2float_rd(y); fr_lo[2] = __double2float_rd(z);
+                have = (x == x) && (y == y) && (z == z);
             }
             if (!((x == x) && (y == y) && (z == z))) atomicOr(P.range_keys + 6, 1u);
         }
         double* g = P.pk + ((size_t)f * (P.frame_slots / kGroup) + slot / kGroup) * kGroupFloats + (slot % kGroup);
         g[0] = x; g[4] = y; g[8] = z;
     }
-    if (P.box_type == BOX_TRI) {
+    {
         __shared__ unsigned int s_keys[6];
         if (threadIdx.x < 6) s_keys[threadIdx.x] = 0u;
         __syncthreads();
 #pragma unroll
         for (int q = 0; q < 3; ++q) {
-            uint32_t kmax = have ? float_key(fr[q]) : 0u, kmin_c = have ? ~float_key(fr[q]) : 0u;
+            uint32_t kmax = have ? float_key(fr[q]) : 0u, kmin_c = have ? ~float_key(fr_lo[q]) : 0u;
             for (int o = 16; o > 0; o >>= 1) {
                 kmax = max(kmax, __shfl_xor_sync(0xffffffffu, kmax, o));
                 kmin_c = max(kmin_c, __shfl_xor_sync(0xffffffffu, kmin_c, o));
@@ -94,6 +103,22 @@ static __global__ void __launch_bounds__(256) repack_kernel_f64(const RepackPara
         __syncthreads();
         if (threadIdx.x < 6 && s_keys[threadIdx.x] != 0u) atomicMax(P.range_keys + threadIdx.x, s_keys[threadIdx.x]);
     }
+}
+
+// No box: an UPPER bound of every pinned d2 of the call in double, from the outward-rounded float bounds of the coordinates
+// (cf. coord_extent2_ru); +inf when a coordinate is NaN.
+__device__ __forceinline__ double coord_extent2_ru64(const unsigned int* __restrict__ keys) {
+    if (__ldg(keys + 6) != 0u) return __longlong_as_double(0x7ff0000000000000ll);
+    double acc = 0.0;
+#pragma unroll
+    for (int q = 0; q < 3; ++q) {
+        const uint32_t kmax = __ldg(keys + q), kmin_c = __ldg(keys + 3 + q);
+        if (kmax != 0u) {
+            const double ext = __dsub_ru((double)key_float(kmax), (double)key_float(~kmin_c));
+            acc = __dadd_ru(acc, __dmul_ru(ext, ext));
+        }
+    }
+    return acc;
 }
 
 // ---- the pinned sequence in double ---------------------------------------------------------------
@@ -143,10 +168,17 @@ __device__ __forceinline__ double pair_d2_f64(double xi, double yi, double zi, d
     return __dadd_rn(__dadd_rn(__dmul_rn(dx, dx), __dmul_rn(dy, dy)), __dmul_rn(dz, dz));
 }
 
-template <int MODE>
+// CLEAN (cdh_sched.cuh KIND_CLEAN, MODE_SHARED): the caller promises that every pair of the stage may be binned where it
+// falls -- no box: d < r_max for every pair (the flushed slots end with the Q3 clamp as usual); orthorhombic full-range
+// histogram: dropped pairs land in slots beyond the flushed ones -- so the DSETP compare and the select are left out.
+template <int MODE, bool CLEAN, bool CLAMP>
 __device__ __forceinline__ void bin_f64(double d2, double rmax, double scale, const HistView& hv, bool keep) {
     const double d = sqrt_rn_f64(d2);
     const uint32_t f = __double2uint_rd(__dmul_rn(d, scale));   // floor, saturating (one F2I)
+    if constexpr (CLEAN && MODE == MODE_SHARED) {
+        hist_inc(hv.hist_addr + 4u * (CLAMP ? min(f, hv.last_bin) : f));
+        return;
+    }
     const uint32_t bin = min(f, hv.last_bin);                   // reading Q3
     const uint32_t b = bin - hv.lo;                             // unsigned wrap for bins below the sweep / window
     bool ok = keep && (d < rmax);                               // false for NaN (NaN input, +inf)
@@ -169,7 +201,7 @@ struct MathF64 {
     using Params = TileParams64;
     static constexpr int kStageBytes = kStageBytes64;
     static constexpr bool kPeriodic = BOX != BOX_NONE;
-    static constexpr bool kHasClean = false;
+    static constexpr bool kHasClean = BOX == BOX_NONE || BOX == BOX_ORTHO;
     static constexpr int kUnroll = 1;
     struct Launch { bool range_ok; bool clean; };
     struct Item {
@@ -181,6 +213,11 @@ struct MathF64 {
     __device__ __forceinline__ static bool launch_begin(const Params& P, Launch& L) {
         L.clean = false;
         L.range_ok = (BOX == BOX_TRI) ? (frac_range(P.range_keys) <= kPruneRange64) : true;
+        // no box: every pinned d is below r_max (sqrt is monotone and correctly rounded) and no coordinate is NaN
+        if constexpr (BOX == BOX_NONE) L.clean = __dsqrt_rn(coord_extent2_ru64(P.range_keys)) < P.rmax;
+        // orthorhombic: the host sized the private histogram for half the box diagonal; the wrapped components stay within
+        // L/2 (1 + 2^-20) while |x / L| < 2^20 (the double product is then exact to 2^-32); no NaN coordinate
+        if constexpr (BOX == BOX_ORTHO) L.clean = P.keep_bins != 0u && __ldg(P.range_keys + 6) == 0u && frac_range(P.range_keys) <= 1048576.0f;
         return true;
     }
     template <int MODE>
@@ -190,6 +227,7 @@ struct MathF64 {
             hv.lim = min(P.smem_bins, P.n_bins - hv.lo);
         } else {
             hv.lo = seg.bin_lo; hv.lim = seg.bin_cnt + seg.last_sweep;
+            if constexpr (BOX == BOX_ORTHO && MODE == MODE_SHARED) if (P.keep_bins != 0u) hv.lim = P.keep_bins;
         }
     }
     __device__ __forceinline__ static void item_begin(const Params&, const Launch& L, const double* __restrict__ g, const Box* s_box,
@@ -221,7 +259,7 @@ struct MathF64 {
                     double d2;
                     if constexpr (PBOX) d2 = pair_d2_f64<BOX>(it.xi[r], it.yi[r], it.zi[r], xj[c], yj[c], zj[c], P.box0, it.ob, it.prune);
                     else d2 = pair_d2_f64<BOX>(it.xi[r], it.yi[r], it.zi[r], xj[c], yj[c], zj[c], *s_box, it.ob, it.prune);
-                    bin_f64<MODE>(d2, P.rmax, P.scale, hv, keep);
+                    bin_f64<MODE, KIND == KIND_CLEAN, BOX == BOX_NONE>(d2, P.rmax, P.scale, hv, keep);
                 }
         }
     }

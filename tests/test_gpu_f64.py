@@ -239,3 +239,37 @@ def test_f64_small_species_take_the_skip_variants(box_type):
     got, info = gpu64(big)
     assert not info["skip"], info
     same(got, oracle64(big), f"f64 large species, box_type {box_type}")
+
+
+def test_f64_clean_forms_and_what_switches_them_off():
+    """The double-precision kernels leave out the d < r_max compare where the call cannot drop a pair (no box: coordinate
+    extent below r_max) or where dropped pairs have slots of their own (orthorhombic full-range histogram); NaN / inf
+    coordinates, r_max inside the extent and inexact scales must fall back or stay exact."""
+    g = np.random.Generator(np.random.PCG64(78))
+    n = 6000
+    base = g.random((n, 3)).astype(np.float32)
+    cases = {"clean": (base, math.sqrt(3.0))}
+    x = base.copy(); x[4321] = x[17]
+    cases["coincident"] = (x, math.sqrt(3.0))
+    x = base.copy(); x[5000, 1] = np.nan
+    cases["nan"] = (x, math.sqrt(3.0))
+    x = base.copy(); x[123, 0] = np.inf
+    cases["inf"] = (x, math.sqrt(3.0))
+    cases["r_max inside the extent"] = (base, 1.2)
+    x = base.copy(); x[0] = (0.0, 0.0, 0.0); x[1] = (1.0, 1.0, 1.0)
+    cases["corner to corner"] = (x, math.sqrt(3.0))            # d = sqrt(3) exactly in double: not below r_max, dropped
+    for name, (pts, r_max) in cases.items():
+        p = inputs.Problem(name, np.ascontiguousarray(pts[None]), np.array([0, 4097, n], dtype=np.int32), inputs.BOX_NONE, None,
+                           r_max, 3000)
+        got, info = gpu64(p)
+        same(got, oracle64(p), f"f64 no box, {name}: {info}")
+    for k, (diag, r_max, n_bins) in enumerate([((10.0, 10.0, 10.0), 5.0, 10000), ((8.0, 9.0, 7.5), 3.75, 3000),
+                                               ((7.3, 8.1, 9.7), 3.65, 7777), ((6.0, 6.0, 6.0), 5.0, 2048)]):
+        p = inputs.uniform_problem(600 + k, (2500, 1700), inputs.BOX_ORTHO, n_bins, r_max, box=np.diag(diag), n_frames=2, spread=1.2)
+        got, info = gpu64(p)
+        same(got, oracle64(p), f"f64 orthorhombic case {k}: {info}")
+        if k == 0:
+            assert info["full_range"]
+            p.coords[1, 77, 0] = np.nan
+            got, info = gpu64(p)
+            same(got, oracle64(p), "f64 orthorhombic full-range histogram with a NaN coordinate")
