@@ -401,7 +401,11 @@ int build_plan(cdh_ctx* ctx, cudaStream_t stream, int32_t n_frames, const int32_
     }
     if (mode != MODE_GLOBAL && smem_bins > cap_ring) n_stages = 2;
     const int smem_bytes = smem_fixed(precision, (int)n_stages) + 4 * ((int)smem_bins + 2);
-    const bool big = 2 * (smem_bytes + 1024) > 228 * 1024 || mode == MODE_HYBRID;          // one CTA per SM
+#ifndef CDH_BIG_BELOW_CTAS
+#define CDH_BIG_BELOW_CTAS 2     // the one-CTA-per-SM shape is taken when fewer than this many 256-thread CTAs fit one SM (measured with 3:
+                                 // config 2 1,309 -> 1,170, config 3 784 -> 694 Gpairs/s: the 1,024-thread shape is bounded to 64 registers)
+#endif
+    const bool big = CDH_BIG_BELOW_CTAS * (smem_bytes + 1024) > 228 * 1024 || mode == MODE_HYBRID;          // one CTA per SM
     const bool skip = !big && mode == MODE_SHARED && !use_simple_only && small_species(off, n_species);
     const int shape = big ? SHAPE_BIG : (skip ? SHAPE_256_SKIP : SHAPE_256);
 
