@@ -167,7 +167,7 @@ const char *cdh_last_error(const cdh_ctx *ctx);
  *   info[6] = kernel variant id (bit 0 fast path, bit 1 double precision, bit 2 global histogram, bit 3 hybrid (shared window of
  *             the bins + L2 updates for the rest), bits 4-7 box type, bits 8-11 form: ORTHO 0 plain /
  *             1 fused / 2 exact-product rint, TRICLINIC zero structure; bit 12 bin-range split, bit 13 one-CTA-per-SM shape,
- *             bit 14 small-species variant: warps skip below-diagonal and padding-only work; bit 15 orthorhombic full-range
+ *             bit 14 small-species variant: warps skip below-diagonal and padding-only work; bit 15 no threshold compare in unpadded stages: orthorhombic full-range
  *             private histogram (a slot for every reachable distance, only the first n_bins flushed); bits 16.. j-chunk size)
  *   info[7] = pair slots the tile kernel is scheduled to walk (evaluated pairs incl. masked and padding lanes)
  * Returns CDH_OK or CDH_ERR_INVALID_ARG. */

@@ -399,6 +399,18 @@ int build_plan(cdh_ctx* ctx, cudaStream_t stream, int32_t n_frames, const int32_
             if (all <= cap_two) { keep_bins = (uint32_t)n_bins; smem_bins = all; }
         }
     }
+    // Triclinic box: the zero-shift candidates reach several r_max, so a slot for every distance does not fit; instead the
+    // CLEAN stages clamp d2 to the threshold (one FMNMX for compare + select, bin_fast2 CLAMP): every dropped pair lands in the
+    // slot of bin(thr2), which must be one of the two spare slots (n_bins, n_bins + 1) and is then not flushed -- so no kept
+    // pair may round up into slot n_bins (reading Q3).  Same two decisive bins as above.
+    if (CDH_ORTHO_CLEAN && !f64 && box_type == CDH_BOX_TRICLINIC && mode == MODE_SHARED && !use_simple_only) {
+        const uint32_t tb = d2_threshold_bits(rmax_f);
+        if (tb < 0x7f800000u) {
+            const float thr2 = bits_f32(tb);
+            const float b_thr = floorf(sqrtf(thr2) * scale_f), b_prev = floorf(sqrtf(std::nextafterf(thr2, 0.0f)) * scale_f);
+            if ((b_thr == (float)n_bins || b_thr == (float)n_bins + 1.0f) && b_prev <= (float)(n_bins - 1)) keep_bins = (uint32_t)n_bins;
+        }
+    }
     if (mode != MODE_GLOBAL && smem_bins > cap_ring) n_stages = 2;
     const int smem_bytes = smem_fixed(precision, (int)n_stages) + 4 * ((int)smem_bins + 2);
 #ifndef CDH_BIG_BELOW_CTAS
@@ -611,7 +623,8 @@ int enqueue_plan(cdh_ctx* ctx, const Plan& pl, const void* coords, cudaStream_t 
         }
         for (size_t k = 0; k < pl.launches.size(); ++k) {
             c.counter = ctx->d_scalars + k;
-            if (!f64) { tp.range_lo = pl.launches[k].lo; tp.range_hi = pl.launches[k].hi; tp.keep_bins = k == 0 ? pl.keep_bins : 0u; }
+            // the orthorhombic full-range form belongs to the first launch (fractional range <= 1.49); the triclinic clamp to both fast ones
+            if (!f64) { tp.range_lo = pl.launches[k].lo; tp.range_hi = pl.launches[k].hi; tp.keep_bins = (k == 0 || (pl.box_type == CDH_BOX_TRICLINIC && k == 1)) ? pl.keep_bins : 0u; }
             void* args[1] = {f64 ? (void*)&tp64 : (void*)&tp};
             CDH_CUDA(cudaLaunchKernel(pl.launches[k].v.fn, dim3(pl.grid), dim3((unsigned)pl.launches[k].v.threads), args,
                                       (size_t)pl.smem_bytes, stream));

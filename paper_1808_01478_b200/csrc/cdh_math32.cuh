@@ -41,7 +41,7 @@ struct MathFast {
     using Params = TileParams;
     static constexpr int kStageBytes = cdh::kStageBytes;
     static constexpr bool kPeriodic = BOX != BOX_NONE;
-    static constexpr bool kHasClean = BOX == BOX_NONE || BOX == BOX_ORTHO;
+    static constexpr bool kHasClean = true;     // no box: coordinate extent; orthorhombic: full-range histogram; triclinic: d2 clamp
     static constexpr int kUnroll = 1;
     static constexpr bool kNoPrune = BOX == BOX_TRI && (TRI & TRI_NOPRUNE) != 0;
     static constexpr int kTri = TRI & ~TRI_NOPRUNE;
@@ -73,6 +73,8 @@ struct MathFast {
             // orthorhombic, fractional range <= 1.49: every wrapped component is within L/2 (1 + 2^-18), so the host could size
             // the private histogram for every reachable distance (keep_bins != 0); no NaN coordinate in the call
             if constexpr (BOX == BOX_ORTHO) L.clean = P.keep_bins != 0u && __ldg(P.range_keys + 6) == 0u;
+            // triclinic: the host found that the slot of bin(thr2) is not a flushed one: dropped pairs are clamped into it
+            if constexpr (BOX == BOX_TRI) L.clean = P.keep_bins != 0u;
         } else {
             L.clean = __float_as_uint(coord_extent2_ru(P.range_keys)) < P.thr2_bits;
         }
@@ -88,7 +90,7 @@ struct MathFast {
             hv.lim = min(P.smem_bins, P.n_bins - hv.lo);
         } else {
             hv.lo = seg.bin_lo; hv.lim = seg.bin_cnt + seg.last_sweep;
-            if constexpr (BOX == BOX_ORTHO && MODE == MODE_SHARED) if (P.keep_bins != 0u) hv.lim = P.keep_bins;   // slots beyond: dropped pairs
+            if constexpr (BOX != BOX_NONE && MODE == MODE_SHARED) if (P.keep_bins != 0u) hv.lim = P.keep_bins;   // slots beyond: dropped pairs
         }
     }
 
@@ -200,7 +202,7 @@ struct MathFast {
             for (int hlf = 0; hlf < 2; ++hlf) {
                 bool k0 = true, k1 = true;
                 if constexpr (MASKED) { k0 = jg + 2 * hlf > ig + r; k1 = jg + 2 * hlf + 1 > ig + r; }
-                bin_fast2<MODE, CLEAN>(D2[r][hlf], k0, k1, L.scale, L.ones.r, P.thr2_bits, it.addr_c, it.sub_c, hv, it.grow);
+                bin_fast2<MODE, CLEAN && (BOX != BOX_TRI || MODE == MODE_SHARED), BOX == BOX_TRI>(D2[r][hlf], k0, k1, L.scale, L.ones.r, P.thr2_bits, it.addr_c, it.sub_c, hv, it.grow);
             }
         }
     }
