@@ -202,6 +202,7 @@ struct MathF64 {
     static constexpr int kStageBytes = kStageBytes64;
     static constexpr bool kPeriodic = BOX != BOX_NONE;
     static constexpr bool kHasClean = BOX == BOX_NONE || BOX == BOX_ORTHO;
+    static constexpr bool kCleanPadded = false;
     static constexpr int kUnroll = 1;
     struct Launch { bool range_ok; bool clean; };
     struct Item {

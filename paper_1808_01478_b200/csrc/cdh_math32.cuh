@@ -42,6 +42,7 @@ struct MathFast {
     static constexpr int kStageBytes = cdh::kStageBytes;
     static constexpr bool kPeriodic = BOX != BOX_NONE;
     static constexpr bool kHasClean = true;     // no box: coordinate extent; orthorhombic: full-range histogram; triclinic: d2 clamp
+    static constexpr bool kCleanPadded = BOX == BOX_TRI;   // the clamp also drops NaN padding, the other two forms must not see any
     static constexpr int kUnroll = 1;
     static constexpr bool kNoPrune = BOX == BOX_TRI && (TRI & TRI_NOPRUNE) != 0;
     static constexpr int kTri = TRI & ~TRI_NOPRUNE;
@@ -216,6 +217,7 @@ struct MathSimple {
     static constexpr int kStageBytes = cdh::kStageBytes;
     static constexpr bool kPeriodic = BOX != BOX_NONE;
     static constexpr bool kHasClean = false;
+    static constexpr bool kCleanPadded = false;
     static constexpr int kUnroll = 1;
     struct Launch { bool clean; };
     using Item = ItemF32;
