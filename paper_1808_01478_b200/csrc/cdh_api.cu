@@ -412,6 +412,14 @@ int build_plan(cdh_ctx* ctx, cudaStream_t stream, int32_t n_frames, const int32_
         }
     }
     if (mode != MODE_GLOBAL && smem_bins > cap_ring) n_stages = 2;
+    if (n_stages > 2 && mode != MODE_GLOBAL) {
+        // two stages instead of four where that lets one more 256-thread CTA fit an SM (config 2's full-range histogram:
+        // 76 KB instead of 82 KB per CTA, 3 instead of 2 CTAs); the depth of the ring itself is worth nothing measurable
+        const int reg_ctas = (f64 || box_type == CDH_BOX_TRICLINIC || use_simple_only) ? 2 : 3;   // what the kernels' registers allow
+        const int per_sm = 228 * 1024;
+        const int b4 = smem_fixed(precision, (int)n_stages) + 4 * ((int)smem_bins + 2) + 1024, b2 = smem_fixed(precision, 2) + 4 * ((int)smem_bins + 2) + 1024;
+        if (std::min(reg_ctas, per_sm / b2) > std::min(reg_ctas, per_sm / b4)) n_stages = 2;
+    }
     const int smem_bytes = smem_fixed(precision, (int)n_stages) + 4 * ((int)smem_bins + 2);
 #ifndef CDH_BIG_BELOW_CTAS
 #define CDH_BIG_BELOW_CTAS 2     // the one-CTA-per-SM shape is taken when fewer than this many 256-thread CTAs fit one SM (measured with 3:
