@@ -191,7 +191,7 @@ __global__ void __launch_bounds__(T, MINB) tile_kernel(const typename M::Params 
             };
             if (stage_masked)
                 body(std::integral_constant<int, KIND_MASKED>{}, (SKIP && ig_warp > jbase) ? min(n_grp, (ig_warp - jbase) >> 2) : 0u);
-            else if (M::kHasClean && L.clean && (M::kCleanPadded || (!i_padded && (n_left & 3u) == 0u)))
+            else if (M::kHasClean && L.clean && (M::kCleanPadded || (!i_padded && (n_left & 3u) == 0u && jbase + n_left <= (uint32_t)seg.nj)))
                 body(std::integral_constant<int, KIND_CLEAN>{}, 0u);
             else
                 body(std::integral_constant<int, KIND_GENERAL>{}, 0u);
