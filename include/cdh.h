@@ -65,7 +65,12 @@ extern "C" {
 #define CDH_FLAG_ACCUMULATE       (1u << 6) /* cdh_histograms ADDS to `out` instead of overwriting it: a caller can feed a
                                               trajectory in chunks of frames (the paper's writer sums every 100 frames,
                                               PAPER.md:338).  Not for cdh_histograms_host (its device result is scratch) */
-#define CDH_FLAG_MAX_SMEM_BINS_SHIFT 8     /* bits 8..31: if non-zero, cap on the bins one CTA keeps in
+#define CDH_FLAG_NO_PDL           (1u << 7) /* launch the tile kernels without programmatic stream serialization (A/B of the
+                                              small-call latency: by default a tile launch starts its prologue while the
+                                              kernel before it still runs and waits on the device before it reads its data) */
+#define CDH_FLAG_NO_ITEM_TABLE    (1u << 8) /* build no per-item descriptor table: the kernel looks every work item up in the
+                                              row / segment tables, as calls with more than 262,144 items do (tests) */
+#define CDH_FLAG_MAX_SMEM_BINS_SHIFT 12    /* bits 12..31: if non-zero, cap on the bins one CTA keeps in
                                               shared memory (forces the bin-range-split path) */
 
 typedef struct cdh_ctx cdh_ctx;  /* opaque; owns device scratch (repacked coordinates, work tables) only */

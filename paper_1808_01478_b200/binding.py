@@ -26,7 +26,9 @@ FLAG_NO_AGGREGATE = 1 << 3
 FLAG_TIME_KERNELS = 1 << 4
 FLAG_GLOBAL_HIST = 1 << 5
 FLAG_ACCUMULATE = 1 << 6
-FLAG_MAX_SMEM_BINS_SHIFT = 8
+FLAG_NO_PDL = 1 << 7
+FLAG_NO_ITEM_TABLE = 1 << 8
+FLAG_MAX_SMEM_BINS_SHIFT = 12
 
 EXPORTS = ["cdh_create", "cdh_histograms", "cdh_histograms_host", "cdh_histograms_stream", "cdh_destroy", "cdh_strerror",
            "cdh_last_error", "cdh_last_call_info", "cdh_call_kernel_ms", "cdh_rdf",

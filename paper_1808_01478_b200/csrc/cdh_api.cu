@@ -32,7 +32,8 @@ struct Plan {
     size_t pk_bytes = 0;                 // repacked coordinates the call needs
     int precision = CDH_F32, box_type = 0, n_hist = 0, n_species = 0, n_frames = 0, n_boxes = 1, n_total = 0;
     uint32_t n_bins = 0, frame_slots = 0, repack_blocks = 0, blocks_per_frame = 0;
-    size_t o_rows = 0, o_boxes = 0, o_off = 0, o_pad = 0, o_rowseg = 0, o_win = 0;
+    size_t o_rows = 0, o_boxes = 0, o_off = 0, o_pad = 0, o_rowseg = 0, o_win = 0, o_desc = 0;
+    bool has_descs = false;
     std::vector<Launch> launches;
     int smem_bytes = 0, mode = MODE_SHARED;
     uint32_t grid = 0, n_items = 0, n_rows = 0, tj = 0, smem_bins = 0, n_stages = 2, keep_bins = 0;
@@ -52,7 +53,12 @@ struct cdh_ctx {
     int max_smem_optin = 0;
     // device scratch, grown on demand, never shrunk
     void* d_pk = nullptr;        size_t pk_bytes = 0;         // repacked coordinates of the call in flight
-    unsigned int* d_scalars = nullptr;                        // [0..2] work counters of the call's tile launches, [4..10] range keys (repack_kernel)
+    // Two sets of 16 words: [0..2] work counters of the call's tile launches, [4..10] range keys (repack_kernel).  Calls take
+    // them in turn and the repack kernel of a call zeroes the set of the NEXT one (every kernel of the previous call, the last
+    // user of that set, is complete by then: same stream), so a call needs no memset node of its own.
+    unsigned int* d_scalars = nullptr;
+    int scalar_set = 0;
+    bool scalars_dirty = false;                               // a call failed half-way: zero both sets before the next one
     void* h_tables = nullptr;    size_t h_tables_bytes = 0;   // pinned staging for a new plan's tables
     cudaEvent_t staged = nullptr;                             // h_tables may be rewritten once this has fired
     bool staged_pending = false;
@@ -139,6 +145,7 @@ bool small_species(const int32_t* off, int32_t n_species) {
 #endif
 constexpr uint64_t kItemsPerCta = CDH_ITEMS_PER_CTA;
 constexpr uint32_t kMinChunk = 32;     // smallest j-chunk (particles)
+constexpr uint64_t kDescItems = 262144;  // calls with at most this many work items get the per-item descriptor table (16 MB)
 #ifndef CDH_STAGES
 #define CDH_STAGES 4           // stages of the TMA ring (cdh_sched.cuh) when the private histogram leaves the room; else 2
 #endif
@@ -191,7 +198,7 @@ extern "C" int cdh_create(cdh_ctx** out, int device, uint32_t flags) {
     ctx->n_sm = prop.multiProcessorCount;
     ctx->max_smem_optin = (int)prop.sharedMemPerBlockOptin;
     DeviceGuard g(device);
-    if (!g.ok || cudaMalloc(&ctx->d_scalars, 64) != cudaSuccess ||
+    if (!g.ok || cudaMalloc(&ctx->d_scalars, 128) != cudaSuccess || cudaMemset(ctx->d_scalars, 0, 128) != cudaSuccess ||
         cudaEventCreateWithFlags(&ctx->staged, cudaEventDisableTiming) != cudaSuccess) {
         cudaGetLastError();
         if (ctx->d_scalars) cudaFree(ctx->d_scalars);
@@ -484,7 +491,7 @@ int build_plan(cdh_ctx* ctx, cudaStream_t stream, int32_t n_frames, const int32_
         // a 2,000-particle frame becomes 94 items of 1024 x 32 pairs instead of 12 of 1024 x 256 (launch-latency regime)
         if (tj <= (uint32_t)kStageParticles && (wt.n_items >= grid_full || tj == kMinChunk)) break;
     }
-    if (wt.n_items >= 0xffffffffull || wt.rows.size() >= 0x7fffffffull) return CDH_ERR_INVALID_ARG;
+    if (wt.n_items >= 0xf0000000ull || wt.rows.size() >= 0x7fffffffull) return CDH_ERR_INVALID_ARG;
     std::vector<int32_t> row_seg((size_t)n_hist, -1);          // first segment of each histogram row (window_kernel)
     for (size_t k = wt.segs.size(); k-- > 0;) row_seg[wt.segs[k].hist] = (int32_t)k;
 
@@ -495,7 +502,10 @@ int build_plan(cdh_ctx* ctx, cudaStream_t stream, int32_t n_frames, const int32_
                  b_rowseg = align256((size_t)n_hist * 4);
     pl->o_rows = b_segs; pl->o_boxes = pl->o_rows + b_rows; pl->o_off = pl->o_boxes + b_boxes; pl->o_pad = pl->o_off + b_off;
     pl->o_rowseg = pl->o_pad + b_off; pl->o_win = pl->o_rowseg + b_rowseg;
-    const size_t tables = pl->o_win + b_rowseg;
+    // one descriptor per item, fetched by the kernel one item ahead (cdh_sched.cuh); calls with very many items do without
+    pl->has_descs = wt.n_items > 0 && wt.n_items <= kDescItems && !(ctx->flags & CDH_FLAG_NO_ITEM_TABLE);
+    pl->o_desc = pl->o_win + b_rowseg;
+    const size_t tables = pl->o_desc + (pl->has_descs ? align256((size_t)wt.n_items * sizeof(ItemDesc)) : 0);
     int rc;
     if (ctx->staged_pending) { CDH_CUDA(cudaEventSynchronize(ctx->staged)); ctx->staged_pending = false; }
     if ((rc = grow(ctx, &ctx->h_tables, &ctx->h_tables_bytes, tables, true)) != CDH_OK) return rc;
@@ -510,6 +520,14 @@ int build_plan(cdh_ctx* ctx, cudaStream_t stream, int32_t n_frames, const int32_
     std::memcpy(h + pl->o_off, off, ((size_t)n_species + 1) * 4);
     std::memcpy(h + pl->o_pad, pad_off.data(), ((size_t)n_species + 1) * 4);
     std::memcpy(h + pl->o_rowseg, row_seg.data(), (size_t)n_hist * 4);
+    if (pl->has_descs) {
+        ItemDesc* dd = reinterpret_cast<ItemDesc*>(h + pl->o_desc);
+        for (size_t r = 0; r + 1 < wt.rows.size(); ++r)
+            for (uint32_t it = wt.rows[r].item_prefix; it < wt.rows[r + 1].item_prefix; ++it) {
+                dd[it].seg = wt.segs[wt.rows[r].seg];
+                dd[it].i0 = wt.rows[r].i0; dd[it].jc = wt.rows[r].jc0 + (it - wt.rows[r].item_prefix); dd[it].pad_[0] = it;
+            }
+    }
     cudaError_t e = cudaEventCreateWithFlags(&pl->uploaded, cudaEventDisableTiming);
     if (e == cudaSuccess) e = cudaMemcpyAsync(pl->d_tables, h, tables, cudaMemcpyHostToDevice, stream);
     if (e == cudaSuccess) e = cudaEventRecord(ctx->staged, stream);
@@ -564,7 +582,10 @@ int enqueue_plan(cdh_ctx* ctx, const Plan& pl, const void* coords, cudaStream_t 
     cudaEvent_t* ev = timing ? ctx->ev + 4 * (ctx->timed_calls % CDH_TIMED_CALLS) : nullptr;
     if (stream != pl.up_stream) CDH_CUDA(cudaStreamWaitEvent(stream, pl.uploaded, 0));   // the tables went up on another stream
     if (timing) CDH_CUDA(cudaEventRecord(ev[0], stream));
-    CDH_CUDA(cudaMemsetAsync(ctx->d_scalars, 0, 64, stream));
+    if (ctx->scalars_dirty) { CDH_CUDA(cudaMemsetAsync(ctx->d_scalars, 0, 128, stream)); ctx->scalar_set = 0; }
+    ctx->scalars_dirty = true;                                   // until this call is enqueued completely
+    unsigned int* scalars = ctx->d_scalars + 16 * ctx->scalar_set;
+    unsigned int* scalars_next = ctx->d_scalars + 16 * (ctx->scalar_set ^ 1);
     const bool zero_out = !(ctx->flags & CDH_FLAG_ACCUMULATE);
     const uint64_t out_count = (uint64_t)pl.n_hist * (uint64_t)pl.n_bins;
     // the repack kernel zeroes the result on its way unless that would be most of its work (few particles, very many bins)
@@ -577,7 +598,7 @@ int enqueue_plan(cdh_ctx* ctx, const Plan& pl, const void* coords, cudaStream_t 
             RepackParams64 rp;
             rp.coords = (const double*)coords; rp.pk = (double*)ctx->d_pk;
             rp.off = (const int32_t*)(d + pl.o_off); rp.pad_off = (const uint32_t*)(d + pl.o_pad);
-            rp.range_keys = ctx->d_scalars + 4; rp.boxes = (const BoxConst64*)(d + pl.o_boxes);
+            rp.range_keys = scalars + 4; rp.reset = scalars_next; rp.boxes = (const BoxConst64*)(d + pl.o_boxes);
             rp.n_species = pl.n_species; rp.n_total = pl.n_total; rp.n_frames = pl.n_frames;
             rp.box_type = pl.box_type; rp.n_boxes = pl.n_boxes;
             rp.frame_slots = pl.frame_slots; rp.blocks_per_frame = pl.blocks_per_frame;
@@ -587,7 +608,7 @@ int enqueue_plan(cdh_ctx* ctx, const Plan& pl, const void* coords, cudaStream_t 
             RepackParams rp;
             rp.coords = (const float*)coords; rp.pk = (float*)ctx->d_pk;
             rp.off = (const int32_t*)(d + pl.o_off); rp.pad_off = (const uint32_t*)(d + pl.o_pad);
-            rp.range_keys = ctx->d_scalars + 4; rp.boxes = (const BoxConst*)(d + pl.o_boxes);
+            rp.range_keys = scalars + 4; rp.reset = scalars_next; rp.boxes = (const BoxConst*)(d + pl.o_boxes);
             rp.n_species = pl.n_species; rp.n_total = pl.n_total; rp.n_frames = pl.n_frames;
             rp.box_type = pl.box_type; rp.n_boxes = pl.n_boxes;
             rp.frame_slots = pl.frame_slots; rp.blocks_per_frame = pl.blocks_per_frame;
@@ -603,7 +624,8 @@ int enqueue_plan(cdh_ctx* ctx, const Plan& pl, const void* coords, cudaStream_t 
         TileParams tp; TileParams64 tp64;
         TileCommon& c = f64 ? static_cast<TileCommon&>(tp64) : static_cast<TileCommon&>(tp);
         c.segs = (const Seg*)d; c.rows = (const Row*)(d + pl.o_rows);
-        c.out = (unsigned long long*)out; c.range_keys = ctx->d_scalars + 4; c.win_lo = (const uint32_t*)(d + pl.o_win);
+        c.descs = pl.has_descs ? (const ItemDesc*)(d + pl.o_desc) : nullptr;
+        c.out = (unsigned long long*)out; c.range_keys = scalars + 4; c.win_lo = (const uint32_t*)(d + pl.o_win);
         c.n_rows = pl.n_rows; c.n_items = pl.n_items; c.n_bins = pl.n_bins; c.tj = pl.tj; c.smem_bins = pl.smem_bins;
         c.n_stages = pl.n_stages;
         if (f64) {
@@ -630,12 +652,20 @@ int enqueue_plan(cdh_ctx* ctx, const Plan& pl, const void* coords, cudaStream_t 
             CDH_CUDA(cudaGetLastError());
         }
         for (size_t k = 0; k < pl.launches.size(); ++k) {
-            c.counter = ctx->d_scalars + k;
+            c.counter = scalars + k;
             // the orthorhombic full-range form belongs to the first launch (fractional range <= 1.49); the triclinic clamp to both fast ones
             if (!f64) { tp.range_lo = pl.launches[k].lo; tp.range_hi = pl.launches[k].hi; tp.keep_bins = (k == 0 || (pl.box_type == CDH_BOX_TRICLINIC && k == 1)) ? pl.keep_bins : 0u; }
             void* args[1] = {f64 ? (void*)&tp64 : (void*)&tp};
-            CDH_CUDA(cudaLaunchKernel(pl.launches[k].v.fn, dim3(pl.grid), dim3((unsigned)pl.launches[k].v.threads), args,
-                                      (size_t)pl.smem_bytes, stream));
+            // programmatic stream serialization: the launch may begin while the kernel before it (repack, window or the
+            // previous tile launch) still runs; the kernel waits (griddepcontrol.wait) before it reads what they wrote
+            cudaLaunchAttribute attr[1];
+            attr[0].id = cudaLaunchAttributeProgrammaticStreamSerialization;
+            attr[0].val.programmaticStreamSerializationAllowed = 1;
+            cudaLaunchConfig_t cfg = {};
+            cfg.gridDim = dim3(pl.grid); cfg.blockDim = dim3((unsigned)pl.launches[k].v.threads);
+            cfg.dynamicSmemBytes = (size_t)pl.smem_bytes; cfg.stream = stream;
+            cfg.attrs = attr; cfg.numAttrs = (ctx->flags & CDH_FLAG_NO_PDL) ? 0 : 1;
+            CDH_CUDA(cudaLaunchKernelExC(&cfg, pl.launches[k].v.fn, args));
         }
     }
     if (timing) {
@@ -644,6 +674,8 @@ int enqueue_plan(cdh_ctx* ctx, const Plan& pl, const void* coords, cudaStream_t 
         ++ctx->timed_calls;
     }
     for (int k = 0; k < 8; ++k) ctx->info[k] = pl.info[k];
+    if (pl.frame_slots > 0) ctx->scalar_set ^= 1;                // the repack kernel has zeroed the other set
+    ctx->scalars_dirty = false;
     return CDH_OK;
 }
 

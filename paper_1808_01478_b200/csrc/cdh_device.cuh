@@ -63,11 +63,21 @@ struct BoxConst {
 };
 static_assert(sizeof(BoxConst) % 16 == 0, "BoxConst is copied and indexed in 16-byte units");
 
+// Everything the scheduler needs to know about one work item, so that a CTA learns it in one (asynchronous) copy instead
+// of four dependent round trips to memory (row search, Row, Seg).  Built by the host unless the call has very many items.
+struct alignas(16) ItemDesc {
+    Seg seg;
+    uint32_t i0, jc;            // first particle of the i-tile inside species p, j-chunk
+    uint32_t pad_[2];           // [0]: the item's index (0xFFFFFFFF in a shared-memory slot: no item left)
+};
+static_assert(sizeof(Seg) == 48 && sizeof(ItemDesc) == 64, "ItemDesc is copied as four 16-byte words");
+
 // The part of the tile kernel's parameters that does not depend on the precision (cdh_sched.cuh).
 struct TileCommon {
     const Seg*      segs;
     const Row*      rows;       // n_rows + 1 entries (last: item_prefix = n_items)
-    unsigned int*   counter;    // dynamic work counter (zeroed before the launch)
+    const ItemDesc* descs;      // n_items entries, or nullptr (calls with very many items look the item up in rows / segs)
+    unsigned int*   counter;    // dynamic work counter of the items past the first one of every CTA (zero before the launch)
     unsigned long long* out;    // uint64 [n_hist][n_bins]
     const unsigned int* range_keys;  // device, written by the repack kernel: [0..2] max keys, [3..5] complemented min keys of the
                                      // fractional coordinates (periodic boxes) or of the raw coordinates (no box), [6] != 0: some
@@ -101,6 +111,18 @@ struct TileParams : TileCommon {
 __device__ __forceinline__ uint32_t smem_u32(const void* p) {
     return static_cast<uint32_t>(__cvta_generic_to_shared(p));
 }
+
+// Programmatic dependent launch (cdh_api.cu launches the tile kernels with programmatic stream serialization): a kernel
+// lets the next one in the stream start its prologue early, and the next one waits here -- for the COMPLETION of every
+// kernel before it -- before it touches anything an earlier kernel of the stream writes.
+__device__ __forceinline__ void pdl_launch_dependents() { asm volatile("griddepcontrol.launch_dependents;" ::: "memory"); }
+__device__ __forceinline__ void pdl_wait() { asm volatile("griddepcontrol.wait;" ::: "memory"); }
+
+// 16-byte asynchronous copy global -> shared (LDGSTS) and the wait for all copies of the executing thread
+__device__ __forceinline__ void cp_async_16(uint32_t dst, const void* src) {
+    asm volatile("cp.async.ca.shared.global [%0], [%1], 16;" ::"r"(dst), "l"(src) : "memory");
+}
+__device__ __forceinline__ void cp_async_wait_all() { asm volatile("cp.async.wait_all;" ::: "memory"); }
 
 __device__ __forceinline__ void mbar_init(uint32_t bar, uint32_t count) {
     asm volatile("mbarrier.init.shared::cta.b64 [%0], %1;" ::"r"(bar), "r"(count));

@@ -40,6 +40,7 @@ struct RepackParams64 {
     const int32_t* off;
     const uint32_t* pad_off;
     unsigned int* range_keys;
+    unsigned int* reset;        // as RepackParams
     const BoxConst64* boxes;
     int32_t n_species, n_total, n_frames;
     int32_t box_type, n_boxes;
@@ -50,6 +51,8 @@ struct RepackParams64 {
 };
 
 static __global__ void __launch_bounds__(256) repack_kernel_f64(const RepackParams64 P) {
+    pdl_launch_dependents();
+    if (blockIdx.x == 0 && threadIdx.x < 16) P.reset[threadIdx.x] = 0u;
     if (P.zero != nullptr)
         for (uint64_t k = (uint64_t)blockIdx.x * 256u + threadIdx.x; k < P.zero_count; k += (uint64_t)gridDim.x * 256u) P.zero[k] = 0ull;
     const uint32_t f = blockIdx.x / P.blocks_per_frame;

@@ -46,6 +46,7 @@ struct RepackParams {
     unsigned int* range_keys;   // device, [7]: atomicMax of key(f_k) (k = 0..2) and of ~key(f_k) (3..5), f = b^-1 x
                                 // (fractional coordinates, approximate; the raw coordinates when there is no box), [6] is set
                                 // when a particle has a NaN coordinate; zero-initialised; see frac_range() / coord_extent2_ru()
+    unsigned int* reset;        // the 16 scalars of the context's NEXT call, zeroed here (cdh_api.cu "d_scalars")
     const BoxConst* boxes;      // box constants (periodic boxes), one or n_frames
     int32_t n_species, n_total, n_frames;
     int32_t box_type, n_boxes;
@@ -99,6 +100,8 @@ __device__ __forceinline__ float coord_extent2_ru(const unsigned int* __restrict
 }
 
 static __global__ void __launch_bounds__(256) repack_kernel(const RepackParams P) {
+    pdl_launch_dependents();    // the tile kernel may start its prologue; it waits for this grid to complete before it reads pk
+    if (blockIdx.x == 0 && threadIdx.x < 16) P.reset[threadIdx.x] = 0u;
     if (P.zero != nullptr)      // saves the call one memset node (small calls are launch-latency bound)
         for (uint64_t k = (uint64_t)blockIdx.x * 256u + threadIdx.x; k < P.zero_count; k += (uint64_t)gridDim.x * 256u) P.zero[k] = 0ull;
     const uint32_t f = blockIdx.x / P.blocks_per_frame;

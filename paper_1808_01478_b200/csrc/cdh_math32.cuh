@@ -106,7 +106,9 @@ struct MathFast {
 #pragma unroll
             for (int k = 0; k < 9; ++k) { it.fb.B[k] = s_box->B[k]; it.fb.Binv[k] = s_box->Binv[k]; }
         }
-        it.addr_c = hv.hist_addr - 4u * (kFloorMagicBits + hv.lo);
+        // pinned in a register each (as grow): where registers are short ptxas otherwise rebuilds the address constant from
+        // the stage count and the CTA's shared window in every group (8 instructions per 16 pairs in the triclinic kernels)
+        asm volatile("mov.b32 %0, %1;" : "=r"(it.addr_c) : "r"(hv.hist_addr - 4u * (kFloorMagicBits + hv.lo)));
         it.sub_c = kFloorMagicBits + hv.lo;
         asm volatile("mov.b64 %0, %1;" : "=l"(it.grow) : "l"(hv.grow));
     }

@@ -24,7 +24,7 @@
 namespace cdh {
 
 constexpr int kR = 4;                       // i-particles per thread (one group)
-constexpr int kSmemHeader = 128;            // 8 mbarriers | scheduler slot | 8 arrival counters
+constexpr int kSmemHeader = 256;            // 8 mbarriers | spare | 8 arrival counters | two work-item descriptors (64 B each)
 constexpr int kMaxStages = 8;
 constexpr uint64_t kMaxIncrements = 0xFFFFFFFFull;
 
@@ -70,10 +70,11 @@ __global__ void __launch_bounds__(T, MINB) tile_kernel(const typename M::Params 
     constexpr uint32_t NW = T / 32;
     constexpr uint32_t kStageBytes = M::kStageBytes;
     constexpr uint32_t kStageReals = kStageGroups * kGroupFloats;
+    constexpr uint32_t kGroupBytes = kStageBytes / kStageGroups;
     const uint32_t NS = P.n_stages;                                  // power of two, 2..8
     uint64_t* bars = reinterpret_cast<uint64_t*>(smem);
-    volatile uint32_t* s_item = reinterpret_cast<volatile uint32_t*>(smem + 64);
     uint32_t* s_cons = reinterpret_cast<uint32_t*>(smem + 96);       // [NS] warp arrivals per stage buffer
+    ItemDesc* s_slot = reinterpret_cast<ItemDesc*>(smem + 128);      // [2] the work item in hand and the next one (thread 0 fills them)
     unsigned char* stage0 = smem + kSmemHeader;
     Box* s_box = reinterpret_cast<Box*>(smem + kSmemHeader + NS * kStageBytes);
     uint32_t* s_hist = reinterpret_cast<uint32_t*>(smem + tile_smem_fixed<M>((int)NS));
@@ -81,21 +82,63 @@ __global__ void __launch_bounds__(T, MINB) tile_kernel(const typename M::Params 
     const uint32_t stage_addr = smem_u32(stage0);
     const int tid = threadIdx.x;
 
+    // Work items.  The first item of a CTA is its own index, the later ones are numbered by the global counter.  Thread 0
+    // fetches item k + 1 WHILE item k is computed: the counter value it needs was requested one item earlier (the atomic
+    // is not waited for until then), and the descriptor travels from the plan's table into the other of two shared-memory
+    // slots as an asynchronous copy, so nothing but one CTA barrier stands between two items (the serial chain atomic ->
+    // row search -> Row -> Seg of the first version cost configs 2-4 1.5-2 %).  Calls with more items than the table holds
+    // look the next item up with ordinary loads at the same point (thread 0's warp then lags by those round trips).
+    // A slot whose index field says kNoItem ends the CTA's loop.
+    constexpr uint32_t kNoItem = 0xFFFFFFFFu;
+    auto fetch_item = [&](const uint32_t item, const uint32_t slot) {
+        ItemDesc* dst = s_slot + slot;
+        if (item >= P.n_items) { dst->pad_[0] = kNoItem; return; }
+        if (P.descs != nullptr) {
+            const uint32_t d = smem_u32(dst);
+            const unsigned char* q = reinterpret_cast<const unsigned char*>(P.descs + item);
+#pragma unroll
+            for (int c = 0; c < 4; ++c) cp_async_16(d + 16u * c, q + 16 * c);
+        } else {
+            uint32_t lo = 0, hi = P.n_rows;         // row of the item: largest r with rows[r].item_prefix <= item
+            while (hi - lo > 1) {
+                const uint32_t mid = (lo + hi) >> 1;
+                if (__ldg(&P.rows[mid].item_prefix) <= item) lo = mid; else hi = mid;
+            }
+            const Row row = P.rows[lo];
+            const uint4* q = reinterpret_cast<const uint4*>(P.segs + row.seg);
+            const uint4 a = __ldg(q), b = __ldg(q + 1), c = __ldg(q + 2);
+            uint4* o = reinterpret_cast<uint4*>(dst);
+            o[0] = a; o[1] = b; o[2] = c;
+            o[3] = make_uint4(row.i0, row.jc0 + (item - row.item_prefix), item, 0u);
+        }
+    };
+
+    // Prologue that reads nothing an earlier kernel of the call writes (the tables are the plan's): it may run while the
+    // repack kernel (or the previous tile launch of the call) is still at work (programmatic dependent launch, cdh_api.cu).
+    pdl_launch_dependents();
+    if (tid == 0) {
+        for (uint32_t k = 0; k < NS; ++k) { mbar_init(bar_addr + 8 * k, 1); s_cons[k] = 0; }
+        fence_mbar_init();
+        fetch_item(blockIdx.x, 0u);
+    }
+    for (uint32_t b = tid; b <= P.smem_bins + 1; b += T) s_hist[b] = 0;
+    pdl_wait();
+
     // Launch gate: the variants of a call own disjoint intervals of a quantity the repack kernel measured on the
     // device (range of the fractional coordinates for periodic boxes) and exactly one of them does the work; the
     // call never synchronises with the host.  Uniform over the grid.
     typename M::Launch L;
     if (!M::launch_begin(P, L)) return;
-
-    if (tid == 0) {
-        for (uint32_t k = 0; k < NS; ++k) { mbar_init(bar_addr + 8 * k, 1); s_cons[k] = 0; }
-        fence_mbar_init();
-    }
-    for (uint32_t b = tid; b <= P.smem_bins + 1; b += T) s_hist[b] = 0;
     HistView hv;
     hv.hist_addr = smem_u32(s_hist);
     hv.trash_addr = hv.hist_addr + 4u * (P.smem_bins + 1u);          // never flushed
     hv.lo = 0; hv.lim = 0; hv.last_bin = P.n_bins - 1u; hv.grow = P.out;
+    const bool one_each = gridDim.x >= P.n_items;      // one CTA per item (small calls): the counter is never touched
+    uint32_t nxt = 0;                                  // thread 0: the counter value that numbers the item to fetch next
+    if (tid == 0) {
+        if (!one_each) nxt = atomicAdd(P.counter, 1u);
+        cp_async_wait_all();
+    }
     __syncthreads();
 
     uint32_t stage_cnt = 0;                 // stages consumed so far: buffer = cnt % NS, parity = (cnt / NS) & 1
@@ -119,24 +162,18 @@ __global__ void __launch_bounds__(T, MINB) tile_kernel(const typename M::Params 
         __syncthreads();
     };
 
-    for (;;) {
-        if (tid == 0) *s_item = atomicAdd(P.counter, 1u);
-        __syncthreads();
-        const uint32_t item = *s_item;
-        if (item >= P.n_items) break;
-
-        // row of the item: largest r with rows[r].item_prefix <= item
-        uint32_t lo = 0, hi = P.n_rows;
-        while (hi - lo > 1) {
-            const uint32_t mid = (lo + hi) >> 1;
-            if (__ldg(&P.rows[mid].item_prefix) <= item) lo = mid; else hi = mid;
+    for (uint32_t k = 0;; ++k) {                       // the item in hand is in slot k & 1
+        const ItemDesc* d = s_slot + (k & 1u);
+        if (d->pad_[0] == kNoItem) break;
+        const Seg seg = d->seg;
+        const uint32_t i0 = d->i0, jc = d->jc;
+        if (tid == 0) {
+            const uint32_t next_item = one_each ? kNoItem : gridDim.x + nxt;
+            fetch_item(next_item, (k + 1u) & 1u);
+            if (next_item < P.n_items) nxt = atomicAdd(P.counter, 1u);
         }
-        const Row row = P.rows[lo];
-        const Seg seg = P.segs[row.seg];
-        const uint32_t jc = row.jc0 + (item - row.item_prefix);
         const uint32_t j0 = jc * P.tj;
         const uint32_t j1 = min((uint32_t)seg.nj, j0 + P.tj);
-        const uint32_t i0 = row.i0;
 
         if (seg.key != cur_key || increments + (uint64_t)TI * P.tj > kMaxIncrements) {
             flush();
@@ -185,9 +222,12 @@ __global__ void __launch_bounds__(T, MINB) tile_kernel(const typename M::Params 
             const bool stage_masked = masked && (jbase < i0 + TI);
             auto body = [&](auto kind_c, const uint32_t g_begin) {
                 constexpr int KIND = decltype(kind_c)::value;
+                // the group's address walks along with g (one add per group; left to itself ptxas rebuilds it from the
+                // stage counter in every iteration where registers are short: triclinic kernels, 6 more instructions)
+                const unsigned char* pg = sj + g_begin * kGroupBytes;
 #pragma unroll M::kUnroll
-                for (uint32_t g = g_begin; g < n_grp; ++g)
-                    M::template group<MODE, KIND>(P, L, it, sj, g, jbase + 4u * g, ig, hv, s_box);
+                for (uint32_t g = g_begin; g < n_grp; ++g, pg += kGroupBytes)
+                    M::template group<MODE, KIND>(P, L, it, pg, 0u, jbase + 4u * g, ig, hv, s_box);
             };
             if (stage_masked)
                 body(std::integral_constant<int, KIND_MASKED>{}, (SKIP && ig_warp > jbase) ? min(n_grp, (ig_warp - jbase) >> 2) : 0u);
@@ -207,7 +247,8 @@ __global__ void __launch_bounds__(T, MINB) tile_kernel(const typename M::Params 
             }
             ++stage_cnt;
         }
-        __syncthreads();              // every warp is done with the item: s_item and the ring are reused
+        if (tid == 0) cp_async_wait_all();
+        __syncthreads();              // every warp is done with the item: the ring is reused, the next item is in its slot
     }
     flush();
 }

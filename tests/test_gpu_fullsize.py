@@ -92,6 +92,13 @@ def test_config3_full(ctx, ctx_simple):
     assert got.sum() / p.evaluated_pairs == pytest.approx(math.pi / 12, rel=2e-3)     # V = d^3 sqrt(2)/2, r = d sqrt(2)/4
 
 
+def test_config3_and_4_full_without_item_table():
+    # the scheduler's other way to learn a work item (row search + Row + Seg instead of the descriptor table), many items per CTA
+    with cdh.Context(0, cdh.FLAG_NO_ITEM_TABLE) as c:
+        for k, p in ((3, inputs.config3()), (4, inputs.config4())):
+            same(run(c, p), golden(k, p)["hist"], f"config {k} without the item table vs the oracle's full-size histogram")
+
+
 def test_config4_full(ctx):
     p = inputs.config4()
     got = run(ctx, p)

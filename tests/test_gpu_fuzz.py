@@ -15,7 +15,8 @@ from oracle import oracle as cdh_oracle
 torch = pytest.importorskip("torch")
 pytestmark = pytest.mark.gpu
 
-FLAGS = [0, 0, 0, cdh.FLAG_NO_PRUNE, cdh.FLAG_SIMPLE_KERNEL, cdh.FLAG_GLOBAL_HIST, 97 << cdh.FLAG_MAX_SMEM_BINS_SHIFT]
+FLAGS = [0, 0, 0, cdh.FLAG_NO_PRUNE, cdh.FLAG_SIMPLE_KERNEL, cdh.FLAG_GLOBAL_HIST, 97 << cdh.FLAG_MAX_SMEM_BINS_SHIFT,
+         cdh.FLAG_NO_ITEM_TABLE, cdh.FLAG_NO_PDL | cdh.FLAG_NO_ITEM_TABLE]
 
 
 def random_problem(g):

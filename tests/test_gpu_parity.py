@@ -63,6 +63,8 @@ FLAG_SETS = {
     "simple_global_hist": cdh.FLAG_GLOBAL_HIST | cdh.FLAG_SIMPLE_KERNEL,
     "match_any": cdh.FLAG_WARP_AGGREGATE,
     "plain_add": cdh.FLAG_NO_AGGREGATE,
+    "no_item_table": cdh.FLAG_NO_ITEM_TABLE,      # every item looked up in the row / segment tables (calls with > 262,144 items)
+    "no_pdl": cdh.FLAG_NO_PDL,                    # tile launches fully serialised behind the repack kernel
 }
 
 
