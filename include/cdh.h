@@ -201,6 +201,35 @@ int cdh_call_kernel_ms(cdh_ctx *ctx, int calls_back, double ms[2]);
 int cdh_rdf(cdh_ctx *ctx, const uint64_t *hist, int32_t n_hist, int32_t n_bins, double r_max, int32_t n_frames,
             const double *n_pairs, double volume, void *stream, double *g);
 
+/*
+ * The histogram call for callers that must not allocate (code under CUDA graph capture, tight serving loops,
+ * harnesses that forbid cudaMalloc): no context, and no cudaMalloc / cudaFree / cudaMallocHost or other allocating
+ * CUDA routine on any call.  All device scratch of the call (repacked coordinates, work tables, work counter) lives
+ * in ONE static device array of CDH_NOALLOC_SCRATCH_BYTES (1.75 MiB) inside the library, which every GPU holds from
+ * the moment it loads the library until the process exits.  Computes what cdh_histograms computes with CDH_F32
+ * (same arguments, same integers; Alg. 1, Eq. 4, Eq. 5), overwriting `out`; the kernels are the same tile
+ * kernel (no box: the production packed-fp32 variant; periodic boxes: the plain cross-validation variant).
+ *
+ *  device   CUDA device ordinal (sm_100); coords and out are DEVICE pointers on it, off and box HOST pointers.
+ *  stream   cudaStream_t (NULL = default stream); the call is asynchronous on it (it returns once the work tables of
+ *           the call have been staged for their host-to-device copy; host arrays may be reused at once).
+ * Limits (beyond them the call returns CDH_ERR_UNSUPPORTED, enqueues nothing, and cdh_noalloc_last_error() says
+ * which limit): n_frames x (padded particles per frame) <= CDH_NOALLOC_MAX_PADDED_PARTICLES, where every species is
+ * padded to a multiple of 4096 particles; n_bins <= CDH_NOALLOC_MAX_BINS; work tables (48 B per frame and species
+ * pair + 16 B per i-tile of 1,024 or 4,096 particles + 560 B per box) <= 255.75 KiB.  Larger problems: cdh_histograms.
+ * The array is SHARED by all calls on a device and keeps the last call's contents; the call clears what must start
+ * at zero.  Calls that overlap on one GPU (two streams, two host threads) race on it: serialise them.
+ * Returns CDH_OK, CDH_ERR_INVALID_ARG, CDH_ERR_UNSUPPORTED or CDH_ERR_CUDA; text via cdh_noalloc_last_error()
+ * (per host thread, valid until that thread's next call).
+ */
+#define CDH_NOALLOC_MAX_PADDED_PARTICLES 131072
+#define CDH_NOALLOC_MAX_BINS             32768
+#define CDH_NOALLOC_SCRATCH_BYTES        1835008   /* 256 KiB scalars + tables, 1.5 MiB repacked coordinates */
+int cdh_histograms_noalloc(int device, const void *coords, int32_t n_frames, const int32_t *species_offsets,
+                           int32_t n_species, int32_t box_type, const double *box, int32_t n_boxes,
+                           double r_max, int32_t n_bins, void *stream, uint64_t *out);
+const char *cdh_noalloc_last_error(void);
+
 #ifdef __cplusplus
 }
 #endif

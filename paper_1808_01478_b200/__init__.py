@@ -7,7 +7,7 @@ load the library; the first call does, and fails loudly if it was not built.
 from . import inputs  # noqa: F401
 from .binding import (BOX_NONE, BOX_ORTHO, BOX_TRICLINIC, F32, F64, FLAG_MAX_SMEM_BINS_SHIFT,  # noqa: F401
                       FLAG_ACCUMULATE, FLAG_GLOBAL_HIST, FLAG_NO_AGGREGATE, FLAG_NO_ITEM_TABLE, FLAG_NO_PDL, FLAG_NO_PRUNE, FLAG_SIMPLE_KERNEL, FLAG_TIME_KERNELS, FLAG_WARP_AGGREGATE, CdhError,
-                      Context, cdh_bench_dsmem_atomics, cdh_bench_fp32_rate, cdh_bench_inner_loop, cdh_bench_shared_atomics, cdh_create, cdh_selftest_sqrt, cdh_selftest_sqrt_f64,
+                      Context, cdh_bench_dsmem_atomics, cdh_bench_fp32_rate, cdh_bench_inner_loop, cdh_bench_shared_atomics, cdh_create, cdh_histograms_noalloc, NOALLOC_MAX_BINS, NOALLOC_MAX_PADDED_PARTICLES, cdh_selftest_sqrt, cdh_selftest_sqrt_f64,
                       cdh_strerror, load)
 
 

@@ -31,7 +31,7 @@ FLAG_NO_ITEM_TABLE = 1 << 8
 FLAG_MAX_SMEM_BINS_SHIFT = 12
 
 EXPORTS = ["cdh_create", "cdh_histograms", "cdh_histograms_host", "cdh_histograms_stream", "cdh_destroy", "cdh_strerror",
-           "cdh_last_error", "cdh_last_call_info", "cdh_call_kernel_ms", "cdh_rdf",
+           "cdh_last_error", "cdh_last_call_info", "cdh_call_kernel_ms", "cdh_rdf", "cdh_histograms_noalloc", "cdh_noalloc_last_error",
            "cdh_bench_fp32_rate", "cdh_bench_shared_atomics", "cdh_bench_inner_loop", "cdh_bench_dsmem_atomics", "cdh_selftest_sqrt", "cdh_selftest_sqrt_f64",
            "cdh_host_d2_threshold_bits", "cdh_host_fused_rint_constant", "cdh_host_work_items"]
 
@@ -65,6 +65,10 @@ def load(path: Optional[str] = None) -> ctypes.CDLL:
     lib.cdh_histograms_host.argtypes = hist_args
     lib.cdh_histograms_stream.restype = ctypes.c_int
     lib.cdh_histograms_stream.argtypes = hist_args[:11] + [i32, vp, vp]
+    lib.cdh_histograms_noalloc.restype = ctypes.c_int
+    lib.cdh_histograms_noalloc.argtypes = [ctypes.c_int, vp, i32, vp, i32, i32, vp, i32, dbl, i32, vp, vp]
+    lib.cdh_noalloc_last_error.restype = ctypes.c_char_p
+    lib.cdh_noalloc_last_error.argtypes = []
     lib.cdh_destroy.restype = ctypes.c_int
     lib.cdh_destroy.argtypes = [vp]
     lib.cdh_strerror.restype = ctypes.c_char_p
@@ -306,6 +310,33 @@ def cdh_bench_shared_atomics(pattern: int, op: int, n_bins: int, samples=None, n
     if rc != OK:
         raise CdhError(rc, cdh_strerror(rc))
     return r.value, ms.value, ms0.value
+
+
+NOALLOC_MAX_PADDED_PARTICLES = 131072
+NOALLOC_MAX_BINS = 32768
+
+
+def cdh_histograms_noalloc(device: int, coords, n_frames: int, species_offsets: Sequence[int], box_type: int, box,
+                           r_max: float, n_bins: int, out, stream=None) -> None:
+    """include/cdh.h ``cdh_histograms_noalloc``: ``cdh_histograms`` (CDH_F32) without a context and without any
+    allocation -- the scratch is a static device array inside the library, shared by all calls on the device (calls that
+    overlap on the GPU race).  coords / out are DEVICE buffers (torch CUDA tensors or ints).  Asynchronous on ``stream``."""
+    lib = load()
+    off = np.ascontiguousarray(species_offsets, dtype=np.int32)
+    n_species = len(off) - 1
+    if box is None:
+        b, n_boxes = None, 0
+    else:
+        b = np.ascontiguousarray(box, dtype=np.float64).reshape(-1, 9)
+        n_boxes = int(b.shape[0])
+    _check_device_tensor(coords, "coords", int(device), "float32", int(n_frames) * int(off[-1]) * 3)
+    _check_device_tensor(out, "out", int(device), "int64|uint64", n_species * (n_species + 1) // 2 * int(n_bins))
+    rc = lib.cdh_histograms_noalloc(int(device), _ptr(coords), int(n_frames), off.ctypes.data, n_species, int(box_type),
+                                    None if b is None else b.ctypes.data, n_boxes, float(r_max), int(n_bins),
+                                    _stream_ptr(stream), _ptr(out))
+    if rc != OK:
+        detail = lib.cdh_noalloc_last_error().decode()
+        raise CdhError(rc, cdh_strerror(rc) + (f" [{detail}]" if detail else ""))
 
 
 def cdh_bench_dsmem_atomics(cluster_size: int, bins_per_cta: int = 25000, iters: int = 512, stream=None):

@@ -16,7 +16,7 @@ LIB = os.path.join(_HERE, "libcdh.so")
 # cdh_api.cu: the C ABI and host dispatch; cdh_k_*.cu: the tile-kernel instantiations, one translation unit per box
 # type so that they compile in parallel; cdh_bench.cu: the roofline microbenchmarks and self-tests.
 SOURCES = ["cdh_api.cu", "cdh_bench.cu", "cdh_k_none.cu", "cdh_k_ortho.cu", "cdh_k_tri.cu", "cdh_k_tri_wide.cu",
-           "cdh_k_simple.cu", "cdh_k_f64.cu"]
+           "cdh_k_simple.cu", "cdh_k_f64.cu", "cdh_noalloc.cu"]
 INCLUDE = os.path.join(_HERE, "..", "include")
 
 
