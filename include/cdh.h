@@ -110,8 +110,11 @@ int cdh_create(cdh_ctx **ctx, int device, uint32_t flags);
  *                      synchronises the DEVICE first (cudaDeviceSynchronize) -- and waits for the previous plan's table
  *                      upload before it reuses the pinned staging buffer.  Do not build plans inside a stream capture.
  *                    - every later call with the same arguments (a trajectory fed frame by frame or chunk by chunk):
- *                      no allocation, no synchronisation, no event wait; it enqueues one memset, the repack kernel
- *                      and the tile kernel launch(es).  The context keeps the 16 most recently used plans.
+ *                      no allocation, no synchronisation, no event wait; it enqueues the repack kernel and the tile
+ *                      kernel launch(es) (and one memset of `out` only when `out` is much larger than the coordinates:
+ *                      otherwise the repack kernel zeroes it).  The tile kernels are launched with programmatic stream
+ *                      serialization: they start while the repack kernel runs and wait on the device before they
+ *                      read its output.  The context keeps the 16 most recently used plans.
  *                  If a plan is used on another stream than the one its tables went up on, the call makes that stream
  *                  wait for the upload (cudaStreamWaitEvent).
  *  out             DEVICE pointer, uint64 [n_species*(n_species+1)/2][n_bins], OVERWRITTEN (added to with

@@ -4,8 +4,8 @@
 // the padded layout, the work tables (uploaded once, into the plan's own device buffer), the kernel variants of the
 // launch plan with their shared-memory sizes and grids.  Plans are cached per context (cdh_ctx::plans, least recently
 // used out), so a trajectory fed frame by frame or chunk by chunk -- the paper's use case, PAPER.md:233, 338 -- pays the
-// host work and the table upload once; a call that hits the cache enqueues one 64-byte memset, the repack kernel and the tile
-// launches and touches no allocator and no event.  All device work of a call is enqueued on the caller's stream.
+// host work and the table upload once; a call that hits the cache enqueues the repack kernel and the tile
+// launches (no memset: the call's scalars are zeroed by the call before it) and touches no allocator and no event.  All device work of a call is enqueued on the caller's stream.
 #include <algorithm>
 #include <cstdio>
 #include <memory>

@@ -4,7 +4,8 @@
 // rule cannot drift between the fp32 and the fp64 kernels.
 //
 // One CTA owns one private uint32 histogram in shared memory (histogram strategy 3, and the
-// paper's shared-memory kernel) and pulls work items (i-tile, j-chunk) from a global counter.
+// paper's shared-memory kernel) and works through work items (i-tile, j-chunk): its own index first, then items numbered
+// by a global counter, each fetched one item ahead ("Work items" below).
 // Items are ordered by (histogram row, bin sweep), so a CTA flushes into the uint64 result only when that key
 // changes, when its increment budget nears 2^32 and at exit.  Each thread keeps R = 4
 // i-particles in registers; the j-chunk streams through a ring of NS shared-memory stages of 256 particles filled
