@@ -627,7 +627,7 @@ int enqueue_plan(cdh_ctx* ctx, const Plan& pl, const void* coords, cudaStream_t 
         c.descs = pl.has_descs ? (const ItemDesc*)(d + pl.o_desc) : nullptr;
         c.out = (unsigned long long*)out; c.range_keys = scalars + 4; c.win_lo = (const uint32_t*)(d + pl.o_win);
         c.n_rows = pl.n_rows; c.n_items = pl.n_items; c.n_bins = pl.n_bins; c.tj = pl.tj; c.smem_bins = pl.smem_bins;
-        c.n_stages = pl.n_stages;
+        c.n_stages = pl.n_stages; c.claim_ahead = (uint64_t)pl.n_items >= 16ull * pl.grid ? 1u : 0u;
         if (f64) {
             tp64.pk = (const double*)ctx->d_pk; tp64.boxes = (const BoxConst64*)(d + pl.o_boxes);
             tp64.rmax = pl.r_max; tp64.scale = (double)pl.n_bins / pl.r_max; tp64.box0 = pl.box0_64; tp64.keep_bins = pl.keep_bins;

@@ -88,6 +88,7 @@ struct TileCommon {
     uint32_t tj;                // j-chunk size in particles (a multiple of kStageParticles, or 32 / 64 / 128 for small calls)
     uint32_t smem_bins;         // capacity of the shared histogram (bins per sweep / window, without the two extra slots)
     uint32_t n_stages;          // stages of the TMA ring (power of two, 2..8)
+    uint32_t claim_ahead;       // SKIP kernels: 1 = a CTA claims its next work item one item early (launches with >= 16 items per CTA)
 };
 
 struct TileParams : TileCommon {

@@ -218,7 +218,7 @@ extern "C" int cdh_histograms_noalloc(int device, const void* coords, int32_t n_
     tp.smem_bins = (uint32_t)n_bins; tp.n_stages = (uint32_t)n_stages;
     tp.pk = d_pk; tp.boxes = (const BoxConst*)(d_tables + o_boxes);
     tp.rmax = rmax_f; tp.scale = scale_f; tp.thr2_bits = d2_threshold_bits(rmax_f); tp.one = 1.0f; tp.one_u = 1.0f;
-    tp.range_lo = -INFINITY; tp.range_hi = INFINITY; tp.keep_bins = 0u;
+    tp.range_lo = -INFINITY; tp.range_hi = INFINITY; tp.keep_bins = 0u; tp.claim_ahead = 1u;
     void* args[1] = {(void*)&tp};
     const uint32_t grid = grid_full < tp.n_items ? grid_full : tp.n_items;
     NA_CUDA(cudaLaunchKernel(v.fn, dim3(grid), dim3((unsigned)v.threads), args, (size_t)smem_bytes, stream));

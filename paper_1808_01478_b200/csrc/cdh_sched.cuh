@@ -135,9 +135,14 @@ __global__ void __launch_bounds__(T, MINB) tile_kernel(const typename M::Params 
     hv.trash_addr = hv.hist_addr + 4u * (P.smem_bins + 1u);          // never flushed
     hv.lo = 0; hv.lim = 0; hv.last_bin = P.n_bins - 1u; hv.grow = P.out;
     const bool one_each = gridDim.x >= P.n_items;      // one CTA per item (small calls): the counter is never touched
+    // Claiming an item one item early costs balance at the end of a launch that gives a CTA only a few items (a CTA holds
+    // an item it will not start for a while; 10,000 points, 2 items per CTA: 986 Gpairs/s claiming ahead, 1,146 claiming
+    // late).  The run-time choice is compiled into the SKIP kernels only -- the ones single frames of small species run --
+    // because the second code path costs the large-problem kernels 1.0-1.7 % (another ptxas schedule of the pair loops).
+    const bool ahead = !SKIP || P.claim_ahead != 0u;
     uint32_t nxt = 0;                                  // thread 0: the counter value that numbers the item to fetch next
     if (tid == 0) {
-        if (!one_each) nxt = atomicAdd(P.counter, 1u);
+        if (!one_each && ahead) nxt = atomicAdd(P.counter, 1u);
         cp_async_wait_all();
     }
     __syncthreads();
@@ -168,7 +173,7 @@ __global__ void __launch_bounds__(T, MINB) tile_kernel(const typename M::Params 
         if (d->pad_[0] == kNoItem) break;
         const Seg seg = d->seg;
         const uint32_t i0 = d->i0, jc = d->jc;
-        if (tid == 0) {
+        if (tid == 0 && ahead) {
             const uint32_t next_item = one_each ? kNoItem : gridDim.x + nxt;
             fetch_item(next_item, (k + 1u) & 1u);
             if (next_item < P.n_items) nxt = atomicAdd(P.counter, 1u);
@@ -248,6 +253,8 @@ __global__ void __launch_bounds__(T, MINB) tile_kernel(const typename M::Params 
             }
             ++stage_cnt;
         }
+        if (SKIP && tid == 0 && !ahead)              // claim as late as possible: both round trips are waited for
+            fetch_item(one_each ? kNoItem : gridDim.x + atomicAdd(P.counter, 1u), (k + 1u) & 1u);
         if (tid == 0) cp_async_wait_all();
         __syncthreads();              // every warp is done with the item: the ring is reused, the next item is in its slot
     }

@@ -79,6 +79,19 @@ def test_reduced_configs_bit_exact(k, variant):
         assert info["sweeps"] == -(-p.n_bins // cap)
 
 
+@pytest.mark.parametrize("counts,n_frames", [((10000,), 1), ((30000,), 1), ((6000, 9000), 3), ((700, 1900), 40)])
+def test_every_pair_once_with_few_and_many_items_per_cta(counts, n_frames):
+    # the scheduler's two ways to claim work (one item ahead; late, where a CTA gets few items) and its two ways to learn an
+    # item (descriptor table; row search): r_max covers the unit cube, so the total must be the closed form (P1),
+    # and all variants must agree bin for bin
+    p = inputs.uniform_problem(4242 + sum(counts), counts, inputs.BOX_NONE, 3000, math.sqrt(3.0) * 1.0001, n_frames=n_frames)
+    got, info = gpu_hist(p)
+    assert int(got.sum()) == p.evaluated_pairs, info
+    assert_same(gpu_hist(p, cdh.FLAG_NO_ITEM_TABLE)[0], got, "row search vs descriptor table")
+    assert_same(gpu_hist(p, cdh.FLAG_NO_PDL)[0], got, "serialised launch vs early launch")
+    assert_same(gpu_hist(p, cdh.FLAG_SIMPLE_KERNEL)[0], got, "cross-validation kernel")
+
+
 def test_config1_full_and_total_count():
     p = inputs.config1()
     got, _ = gpu_hist(p)
