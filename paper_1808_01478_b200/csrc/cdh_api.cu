@@ -428,11 +428,17 @@ int build_plan(cdh_ctx* ctx, cudaStream_t stream, int32_t n_frames, const int32_
         if (std::min(reg_ctas, per_sm / b2) > std::min(reg_ctas, per_sm / b4)) n_stages = 2;
     }
     const int smem_bytes = smem_fixed(precision, (int)n_stages) + 4 * ((int)smem_bins + 2);
+#ifndef CDH_BIG_BELOW_CTAS_NONE
+#define CDH_BIG_BELOW_CTAS_NONE 3
+#endif
 #ifndef CDH_BIG_BELOW_CTAS
 #define CDH_BIG_BELOW_CTAS 2     // the one-CTA-per-SM shape is taken when fewer than this many 256-thread CTAs fit one SM (measured with 3:
                                  // config 2 1,309 -> 1,170, config 3 784 -> 694 Gpairs/s: the 1,024-thread shape is bounded to 64 registers)
 #endif
-    const bool big = CDH_BIG_BELOW_CTAS * (smem_bytes + 1024) > 228 * 1024 || mode == MODE_HYBRID;          // one CTA per SM
+    // no box: the 1,024-thread kernel needs 62 registers and loses nothing to the cap of 64, so it is also taken where only two
+    // 256-thread CTAs (16 warps per SM instead of 32) would fit (measured, 25,000 bins: 2,040 -> 2,111 Gpairs/s)
+    const int big_below = (box_type == CDH_BOX_NONE && !f64 && !use_simple_only) ? CDH_BIG_BELOW_CTAS_NONE : CDH_BIG_BELOW_CTAS;
+    const bool big = big_below * (smem_bytes + 1024) > 228 * 1024 || mode == MODE_HYBRID;          // one CTA per SM
     const bool skip = !big && mode == MODE_SHARED && !use_simple_only && small_species(off, n_species);
     const int shape = big ? SHAPE_BIG : (skip ? SHAPE_256_SKIP : SHAPE_256);
 
