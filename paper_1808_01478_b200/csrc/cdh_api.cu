@@ -141,7 +141,10 @@ bool small_species(const int32_t* off, int32_t n_species) {
 }
 
 #ifndef CDH_ITEMS_PER_CTA
-#define CDH_ITEMS_PER_CTA 64   // work items per resident CTA the j-chunk size is shrunk for (tail of the dynamic schedule)
+#define CDH_ITEMS_PER_CTA 128  // work items per resident CTA the j-chunk size is shrunk for (tail of the dynamic schedule).  Measured
+                               // with the item hand-over down to one CTA barrier: 16 / 32 / 64 / 128 / 256 give config 4 1,344 / 1,374 /
+                               // 1,385 / 1,388 / 1,385 and config 5 2,191 / 2,191 / 2,191 / 2,201 / 2,203 Gpairs/s (configs 2 and 3 sit at
+                               // the smallest j-chunk of a large call, one stage, from 64 on)
 #endif
 constexpr uint64_t kItemsPerCta = CDH_ITEMS_PER_CTA;
 constexpr uint32_t kMinChunk = 32;     // smallest j-chunk (particles)

@@ -177,7 +177,7 @@ extern "C" int cdh_histograms_noalloc(int device, const void* coords, int32_t n_
     uint32_t tj = 8192;
     for (;; tj >>= 1) {
         build_tables(n_frames, off, n_species, nb > 0 ? nb : 1, (uint32_t)n_bins, sp, ti, tj, pad_off, frame_slots, &wt);
-        if (wt.n_items >= 64ull * grid_full) break;
+        if (wt.n_items >= 128ull * grid_full) break;
         if (tj <= (uint32_t)kStageParticles && (wt.n_items >= grid_full || tj == 32u)) break;
     }
     if (wt.n_items >= 0xf0000000ull) return fail(CDH_ERR_INVALID_ARG, "too many work items");
