@@ -442,7 +442,12 @@ int build_plan(cdh_ctx* ctx, cudaStream_t stream, int32_t n_frames, const int32_
     // 256-thread CTAs (16 warps per SM instead of 32) would fit (measured, 25,000 bins: 2,040 -> 2,111 Gpairs/s)
     const int big_below = (box_type == CDH_BOX_NONE && !f64 && !use_simple_only) ? CDH_BIG_BELOW_CTAS_NONE : CDH_BIG_BELOW_CTAS;
     const bool big = big_below * (smem_bytes + 1024) > 228 * 1024 || mode == MODE_HYBRID;          // one CTA per SM
-    const bool skip = !big && mode == MODE_SHARED && !use_simple_only && small_species(off, n_species);
+    // the SKIP kernels also carry the late claim of work items (cdh_sched.cuh), which pays where a CTA gets only a few items:
+    // they are taken as well when the call has fewer than about 6 one-stage items per resident CTA (measured, single frames,
+    // calls back to back: 20,000 points no box 1,267 -> 1,412, orthorhombic 851 -> 1,044; 30,000 points triclinic 710 -> 761;
+    // 40,000 points, 7 items per CTA: -0.6 / -2.5 / +1.3 %, left alone)
+    const bool few_items = frame_pairs(off, n_species) * (double)n_frames < 6.0 * 3.0 * (double)ctx->n_sm * 1024.0 * (double)kStageParticles;
+    const bool skip = !big && mode == MODE_SHARED && !use_simple_only && (small_species(off, n_species) || few_items);
     const int shape = big ? SHAPE_BIG : (skip ? SHAPE_256_SKIP : SHAPE_256);
 
     // ---- launch plan ----------------------------------------------------------------------------
