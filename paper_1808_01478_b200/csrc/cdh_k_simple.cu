@@ -6,8 +6,8 @@ namespace cdh {
 template <int VAR>
 static Variant simple_of(int box, int mode, int shape) {
     if (box == BOX_NONE) return shapes_of<MathSimple<BOX_NONE, VAR>, 2, CDH_BIG_T, false>(mode, shape);
-    if (box == BOX_ORTHO) return shapes_of<MathSimple<BOX_ORTHO, VAR>, 2, CDH_BIG_T, false>(mode, shape);
-    return shapes_of<MathSimple<BOX_TRI, VAR>, 2, CDH_BIG_T, false>(mode, shape);
+    if (box == BOX_ORTHO) return shapes_of<MathSimple<BOX_ORTHO, VAR>, 2, CDH_BIG_T_PERIODIC, false, CDH_HYB_T_ORTHO>(mode, shape);
+    return shapes_of<MathSimple<BOX_TRI, VAR>, 2, CDH_BIG_T_PERIODIC, false>(mode, shape);
 }
 Variant simple_variant(int box, int var, int mode, int shape) {
     if (var == VAR_SIMPLE_MATCH && mode == MODE_SPLIT) return simple_of<VAR_SIMPLE_MATCH>(box, mode, shape);

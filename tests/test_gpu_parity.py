@@ -266,6 +266,21 @@ def test_hybrid_window_single_sweep(n_bins, box_type):
         assert int(got.sum()) == 12_000 * 11_999 // 2
 
 
+@pytest.mark.parametrize("box_type", [inputs.BOX_ORTHO, inputs.BOX_TRICLINIC])
+@pytest.mark.parametrize("n_bins", [40_000, 70_000])
+@pytest.mark.parametrize("spread", [1.0, 5.0, 200.0, 3.0e6])
+def test_one_cta_per_sm_plans_in_every_range_tier(box_type, n_bins, spread):
+    """40,000 bins: one 512-thread CTA per SM (periodic boxes); 70,000 bins: the hybrid plans (1,024 threads orthorhombic, 512
+    triclinic).  The work tables of a plan are built for ONE i-tile size, so the launch that owns the measured coordinate range
+    -- fast narrow form, wide / plain-rint form, or the cross-validation kernel far outside -- must have the CTA size of the
+    plan's first launch.  Coordinates inside the cell, a few cells away, hundreds of cells away, millions of cells away."""
+    box = np.diag([5.0, 6.0, 7.0]) if box_type == inputs.BOX_ORTHO else np.array([[6.0, 0.0, 0.0], [1.0, 5.5, 0.0], [-0.5, 1.5, 5.0]])
+    p = inputs.uniform_problem(int(n_bins + spread) % 9973, (1300, 2900), box_type, n_bins, 2.4, box=box, spread=spread)
+    got, info = gpu_hist(p)
+    assert info["ctas"] <= 148 and info["threads"] in (512, 1024) and info["hybrid"] == (n_bins > 56_402), info
+    assert_same(got, oracle_hist(p), f"{n_bins} bins, box {box_type}, spread {spread}: {info}")
+
+
 def test_empty_species_tiny_inputs_and_nan():
     pts = np.array([[0.1, 0.2, 0.3], [0.5, 0.5, 0.5], [np.nan, 0.0, 0.0], [0.9, 0.1, 0.4]], dtype=np.float32)[None]
     p = inputs.Problem("tiny", pts, np.array([0, 0, 1, 1, 4], dtype=np.int32), inputs.BOX_NONE, None, 2.0, 7)
