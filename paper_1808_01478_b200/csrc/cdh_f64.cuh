@@ -246,7 +246,7 @@ struct MathF64 {
             for (int k = 0; k < 3; ++k) { it.ob.L[k] = s_box->L[k]; it.ob.invL[k] = s_box->invL[k]; }
         }
     }
-    template <int MODE, int KIND>
+    template <int MODE, int KIND, bool SKIPV = false>
     __device__ __forceinline__ static void group(const Params& P, const Launch&, const Item& it, const unsigned char* stage,
                                                  uint32_t g, uint32_t jg, uint32_t ig, const HistView& hv, const Box* s_box) {
         constexpr bool MASKED = KIND == KIND_MASKED;

@@ -34,6 +34,14 @@ __device__ __forceinline__ void load_i_group(const float* __restrict__ g, ItemF3
 // pruning").  A kernel of its own so that the pruned kernel does not pay its registers (config 3: 76 bytes of spills).
 constexpr int TRI_NOPRUNE = 8;
 
+#ifndef CDH_TRI_FIXUP
+#define CDH_TRI_FIXUP 4   // bit k: the narrow-range triclinic form k (TRI_GENERAL 0, TRI_UPPER 1, TRI_UPPER_B01 2) of the large-problem
+                          // kernels bins first and moves the rare pair later.  Measured, 100,000 points: form 2 (config 3's) 821 -> 848
+                          // Gpairs/s (ptxas parks the j-group in uniform registers across phase 2 and reads it from there in phase 1,
+                          // and nothing of the rare path is merged back into the common one); form 0 656 -> 640, form 1 804 -> 774 and
+                          // the SKIP kernels 508 -> 459 (they spill): left as they were
+#endif
+
 template <int BOX, int TRI>
 struct MathFast {
     using Real = float;
@@ -113,11 +121,12 @@ struct MathFast {
         asm volatile("mov.b64 %0, %1;" : "=l"(it.grow) : "l"(hv.grow));
     }
 
-    template <int MODE, int KIND>
+    template <int MODE, int KIND, bool SKIPV = false>
     __device__ __forceinline__ static void group(const Params& P, const Launch& L, const Item& it, const unsigned char* stage,
                                                  uint32_t g, uint32_t jg, uint32_t ig, const HistView& hv, const Box* s_box) {
         constexpr bool MASKED = KIND == KIND_MASKED;
         constexpr bool CLEAN = KIND == KIND_CLEAN && (MODE == MODE_SHARED || MODE == MODE_HYBRID || MODE == MODE_GLOBAL);
+        constexpr bool FIXUP = BOX == BOX_TRI && MODE == MODE_SHARED && !SKIPV && (kTri & TRI_WIDE) == 0 && (CDH_TRI_FIXUP & (1 << (kTri & 3))) != 0;
         const float4* sj = reinterpret_cast<const float4*>(stage);
         const float4 XJ = sj[3 * g], YJ = sj[3 * g + 1], ZJ = sj[3 * g + 2];
         const f2 XA = pk2(XJ.x, XJ.y), XB = pk2(XJ.z, XJ.w), YA = pk2(YJ.x, YJ.y), YB = pk2(YJ.z, YJ.w),
@@ -145,7 +154,49 @@ struct MathFast {
                     if constexpr (BOX == BOX_TRI) fm_all = fmaxf(fmaxf(fm_all, f0), f1);
                 }
             }
-            if constexpr (BOX == BOX_TRI) {
+            if constexpr (FIXUP) {
+                // Shared-memory histogram: bin the whole group first, with the d2 of the first-guess image, and MOVE the rare
+                // pair the neighbour search corrects afterwards (-1 on the slot it went to, +1 on the right one).  The common
+                // path then carries nothing of the rare one: corrected values merged back into D2 cost it 12 MOV per group.
+                constexpr bool CLEANF = CLEAN;
+#pragma unroll
+                for (int r = 0; r < kR; ++r) {
+#pragma unroll
+                    for (int hlf = 0; hlf < 2; ++hlf) {
+                        bool k0 = true, k1 = true;
+                        if constexpr (MASKED) { k0 = jg + 2 * hlf > ig + r; k1 = jg + 2 * hlf + 1 > ig + r; }
+                        bin_fast2<MODE, CLEANF, true>(D2[r][hlf], k0, k1, L.scale, L.ones.r, P.thr2_bits, it.addr_c, it.sub_c, hv, it.grow);
+                    }
+                }
+                if (fm_all > L.prune_lim) {
+                    const float xj[4] = {XJ.x, XJ.y, XJ.z, XJ.w}, yj[4] = {YJ.x, YJ.y, YJ.z, YJ.w}, zj[4] = {ZJ.x, ZJ.y, ZJ.z, ZJ.w};
+#pragma unroll
+                    for (int r = 0; r < kR; ++r) {
+#pragma unroll
+                        for (int hlf = 0; hlf < 2; ++hlf) {
+                            float xr = it.xi[r], f0, f1;
+                            asm volatile("" : "+f"(xr));                 // opaque: recomputed here, nothing of phase 1 is kept alive
+                            const f2 d2f = pair_d2_fast<BOX, kTri>(hlf ? XB : XA, hlf ? YB : YA, hlf ? ZB : ZA, xr, it.yi[r], it.zi[r], it.fb, L.ones, f0, f1);
+                            float pf, qf; upk2(d2f, pf, qf);
+                            bool k0 = true, k1 = true;
+                            if constexpr (MASKED) { k0 = jg + 2 * hlf > ig + r; k1 = jg + 2 * hlf + 1 > ig + r; }
+                            if (f0 > L.prune_lim && k0) {
+                                const float pe = tri_full_d2(it.xi[r], it.yi[r], it.zi[r], xj[2 * hlf], yj[2 * hlf], zj[2 * hlf], s_box);
+                                const uint32_t a_old = bin_addr_shared<CLEANF, true>(pf, k0, L.scale, L.ones.r, P.thr2_bits, it.addr_c, hv);
+                                const uint32_t a_new = bin_addr_shared<CLEANF, true>(pe, k0, L.scale, L.ones.r, P.thr2_bits, it.addr_c, hv);
+                                if (a_old != a_new) { hist_add(a_old, 0xFFFFFFFFu); hist_inc(a_new); }
+                            }
+                            if (f1 > L.prune_lim && k1) {
+                                const float qe = tri_full_d2(it.xi[r], it.yi[r], it.zi[r], xj[2 * hlf + 1], yj[2 * hlf + 1], zj[2 * hlf + 1], s_box);
+                                const uint32_t a_old = bin_addr_shared<CLEANF, true>(qf, k1, L.scale, L.ones.r, P.thr2_bits, it.addr_c, hv);
+                                const uint32_t a_new = bin_addr_shared<CLEANF, true>(qe, k1, L.scale, L.ones.r, P.thr2_bits, it.addr_c, hv);
+                                if (a_old != a_new) { hist_add(a_old, 0xFFFFFFFFu); hist_inc(a_new); }
+                            }
+                        }
+                    }
+                }
+                return;
+            } else if constexpr (BOX == BOX_TRI) {
                 if (fm_all > L.prune_lim) {
                     const float xj[4] = {XJ.x, XJ.y, XJ.z, XJ.w}, yj[4] = {YJ.x, YJ.y, YJ.z, YJ.w}, zj[4] = {ZJ.x, ZJ.y, ZJ.z, ZJ.w};
 #pragma unroll
@@ -240,7 +291,7 @@ struct MathSimple {
                                                       const HistView&, Item& it) {
         load_i_group(gi, it);
     }
-    template <int MODE, int KIND>
+    template <int MODE, int KIND, bool SKIPV = false>
     __device__ __forceinline__ static void group(const Params& P, const Launch&, const Item& it, const unsigned char* stage,
                                                  uint32_t g, uint32_t jg, uint32_t ig, const HistView& hv, const Box* s_box) {
         constexpr bool MASKED = KIND == KIND_MASKED;

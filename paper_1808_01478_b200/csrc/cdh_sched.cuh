@@ -233,7 +233,7 @@ __global__ void __launch_bounds__(T, MINB) tile_kernel(const typename M::Params 
                 const unsigned char* pg = sj + g_begin * kGroupBytes;
 #pragma unroll M::kUnroll
                 for (uint32_t g = g_begin; g < n_grp; ++g, pg += kGroupBytes)
-                    M::template group<MODE, KIND>(P, L, it, pg, 0u, jbase + 4u * g, ig, hv, s_box);
+                    M::template group<MODE, KIND, SKIP>(P, L, it, pg, 0u, jbase + 4u * g, ig, hv, s_box);
             };
             if (stage_masked)
                 body(std::integral_constant<int, KIND_MASKED>{}, (SKIP && ig_warp > jbase) ? min(n_grp, (ig_warp - jbase) >> 2) : 0u);
