@@ -473,6 +473,25 @@ def test_triclinic_pairs_on_the_half_cell_switch_points(r_max):
         assert_same(got, want, f"flags {flags:#x} {info}")
 
 
+def test_triclinic_rare_pairs_in_the_large_problem_kernel():
+    """The large-problem kernel of the TRI_UPPER_B01 form bins a group first and MOVES the rare pair the neighbour search
+    corrects afterwards (csrc/cdh_math32.cuh, CDH_TRI_FIXUP).  Half of the points sit within a few ulps of the half-cell
+    lattice of a dyadic cell, so that a large share of the pairs -- in diagonal (masked), full and ragged stages -- has a
+    fractional separation at the switch point 1/2; big enough for the large-problem kernel (not the SKIP one)."""
+    box = np.array([[16.0, 0.0, 0.0], [0.0, 16.0, 0.0], [8.0, 8.0, 16.0]])        # heights 14.3, 14.3, 16; B upper triangular, B01 = 0
+    g = np.random.Generator(np.random.PCG64(424242))
+    n, f = 26_000, 3
+    frac = g.random((f, n, 3))
+    lattice = g.integers(0, 2, size=(f, n // 2, 3)) * 0.5 + g.integers(-8, 9, size=(f, n // 2, 3)) * 2.0 ** -23
+    frac[:, : n // 2] = lattice
+    coords = (frac @ box).astype(np.float32)
+    p = inputs.Problem("tri_rare_large", coords, np.array([0, n], dtype=np.int32), inputs.BOX_TRICLINIC, box.reshape(1, 9), 7.0, 20_000)
+    got, info = gpu_hist(p)
+    assert not info["skip"] and info["form"] == 2 and info["threads"] == 256, info
+    assert_same(got, oracle_hist(p), f"rare pairs, large-problem kernel: {info}")
+    assert_same(gpu_hist(p, cdh.FLAG_NO_PRUNE)[0], got, "27-shift search for every pair")
+
+
 @pytest.mark.parametrize("box_type", [inputs.BOX_NONE, inputs.BOX_ORTHO, inputs.BOX_TRICLINIC])
 def test_small_species_take_the_skip_variants(box_type):
     # species of a few i-tiles each: the launch plan takes the kernels whose warps skip the j-groups below the diagonal
