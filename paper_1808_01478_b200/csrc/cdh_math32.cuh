@@ -34,6 +34,9 @@ __device__ __forceinline__ void load_i_group(const float* __restrict__ g, ItemF3
 // pruning").  A kernel of its own so that the pruned kernel does not pay its registers (config 3: 76 bytes of spills).
 constexpr int TRI_NOPRUNE = 8;
 
+#ifndef CDH_TRI_FIXUP_WIDE
+#define CDH_TRI_FIXUP_WIDE 0   // ... and not in the wide-range forms (config 3 shifted by up to 3 cells: 633 -> 621 Gpairs/s with it)
+#endif
 #ifndef CDH_TRI_FIXUP
 #define CDH_TRI_FIXUP 4   // bit k: the narrow-range triclinic form k (TRI_GENERAL 0, TRI_UPPER 1, TRI_UPPER_B01 2) of the large-problem
                           // kernels bins first and moves the rare pair later.  Measured, 100,000 points: form 2 (config 3's) 821 -> 848
@@ -126,7 +129,7 @@ struct MathFast {
                                                  uint32_t g, uint32_t jg, uint32_t ig, const HistView& hv, const Box* s_box) {
         constexpr bool MASKED = KIND == KIND_MASKED;
         constexpr bool CLEAN = KIND == KIND_CLEAN && (MODE == MODE_SHARED || MODE == MODE_HYBRID || MODE == MODE_GLOBAL);
-        constexpr bool FIXUP = BOX == BOX_TRI && MODE == MODE_SHARED && !SKIPV && (kTri & TRI_WIDE) == 0 && (CDH_TRI_FIXUP & (1 << (kTri & 3))) != 0;
+        constexpr bool FIXUP = BOX == BOX_TRI && MODE == MODE_SHARED && !SKIPV && (CDH_TRI_FIXUP_WIDE || (kTri & TRI_WIDE) == 0) && (CDH_TRI_FIXUP & (1 << (kTri & 3))) != 0;
         const float4* sj = reinterpret_cast<const float4*>(stage);
         const float4 XJ = sj[3 * g], YJ = sj[3 * g + 1], ZJ = sj[3 * g + 2];
         const f2 XA = pk2(XJ.x, XJ.y), XB = pk2(XJ.z, XJ.w), YA = pk2(YJ.x, YJ.y), YB = pk2(YJ.z, YJ.w),
