@@ -109,6 +109,10 @@ int cdh_create(cdh_ctx **ctx, int device, uint32_t flags);
  *                      may grow the context's scratch -- growing a buffer that enqueued work may still read
  *                      synchronises the DEVICE first (cudaDeviceSynchronize) -- and waits for the previous plan's table
  *                      upload before it reuses the pinned staging buffer.  Do not build plans inside a stream capture.
+ *                      A call that hits the plan cache MAY be captured into a CUDA graph (cudaStreamBeginCapture ...) and
+ *                      replayed any number of times, also between other calls of the context: make the first call with
+ *                      these arguments, and synchronise its stream, before the capture begins; a context created with
+ *                      CDH_FLAG_TIME_KERNELS records events and cannot be captured.
  *                    - every later call with the same arguments (a trajectory fed frame by frame or chunk by chunk):
  *                      no allocation, no synchronisation, no event wait; it enqueues the repack kernel and the tile
  *                      kernel launch(es) (and one memset of `out` only when `out` is much larger than the coordinates:

@@ -53,9 +53,11 @@ struct cdh_ctx {
     int max_smem_optin = 0;
     // device scratch, grown on demand, never shrunk
     void* d_pk = nullptr;        size_t pk_bytes = 0;         // repacked coordinates of the call in flight
-    // Two sets of 16 words: [0..2] work counters of the call's tile launches, [4..10] range keys (repack_kernel).  Calls take
-    // them in turn and the repack kernel of a call zeroes the set of the NEXT one (every kernel of the previous call, the last
-    // user of that set, is complete by then: same stream), so a call needs no memset node of its own.
+    // Four sets of 16 words: [0..2] work counters of the call's tile launches, [4..10] range keys (repack_kernel).  Calls take
+    // sets 0 and 1 in turn and the repack kernel of a call zeroes the set of the NEXT one (every kernel of the previous call, the
+    // last user of that set, is complete by then: same stream), so a call needs no memset node of its own.
+    // A call enqueued while its stream is being CAPTURED into a CUDA graph may be replayed any number of times, between other
+    // calls: it uses set 2, zeroed by a memset node of its own, and aims the repack kernel's zeroing at set 3 (a dummy).
     unsigned int* d_scalars = nullptr;
     int scalar_set = 0;
     bool scalars_dirty = false;                               // a call failed half-way: zero both sets before the next one
@@ -201,7 +203,7 @@ extern "C" int cdh_create(cdh_ctx** out, int device, uint32_t flags) {
     ctx->n_sm = prop.multiProcessorCount;
     ctx->max_smem_optin = (int)prop.sharedMemPerBlockOptin;
     DeviceGuard g(device);
-    if (!g.ok || cudaMalloc(&ctx->d_scalars, 128) != cudaSuccess || cudaMemset(ctx->d_scalars, 0, 128) != cudaSuccess ||
+    if (!g.ok || cudaMalloc(&ctx->d_scalars, 256) != cudaSuccess || cudaMemset(ctx->d_scalars, 0, 256) != cudaSuccess ||
         cudaEventCreateWithFlags(&ctx->staged, cudaEventDisableTiming) != cudaSuccess) {
         cudaGetLastError();
         if (ctx->d_scalars) cudaFree(ctx->d_scalars);
@@ -594,12 +596,21 @@ int enqueue_plan(cdh_ctx* ctx, const Plan& pl, const void* coords, cudaStream_t 
     char* d = (char*)pl.d_tables;
     const bool timing = ctx->ev != nullptr;
     cudaEvent_t* ev = timing ? ctx->ev + 4 * (ctx->timed_calls % CDH_TIMED_CALLS) : nullptr;
-    if (stream != pl.up_stream) CDH_CUDA(cudaStreamWaitEvent(stream, pl.uploaded, 0));   // the tables went up on another stream
+    cudaStreamCaptureStatus cap_status = cudaStreamCaptureStatusNone;
+    CDH_CUDA(cudaStreamIsCapturing(stream, &cap_status));
+    const bool capturing = cap_status == cudaStreamCaptureStatusActive;   // the call is being recorded into a CUDA graph
+    // the tables went up on another stream (under capture the caller has seen to it: include/cdh.h)
+    if (stream != pl.up_stream && !capturing) CDH_CUDA(cudaStreamWaitEvent(stream, pl.uploaded, 0));
     if (timing) CDH_CUDA(cudaEventRecord(ev[0], stream));
-    if (ctx->scalars_dirty) { CDH_CUDA(cudaMemsetAsync(ctx->d_scalars, 0, 128, stream)); ctx->scalar_set = 0; }
-    ctx->scalars_dirty = true;                                   // until this call is enqueued completely
-    unsigned int* scalars = ctx->d_scalars + 16 * ctx->scalar_set;
-    unsigned int* scalars_next = ctx->d_scalars + 16 * (ctx->scalar_set ^ 1);
+    unsigned int* scalars; unsigned int* scalars_next;
+    if (capturing) {
+        scalars = ctx->d_scalars + 32; scalars_next = ctx->d_scalars + 48;
+        CDH_CUDA(cudaMemsetAsync(scalars, 0, 64, stream));       // a node of the graph: every replay starts from zero
+    } else {
+        if (ctx->scalars_dirty) { CDH_CUDA(cudaMemsetAsync(ctx->d_scalars, 0, 128, stream)); ctx->scalar_set = 0; }
+        ctx->scalars_dirty = true;                               // until this call is enqueued completely
+        scalars = ctx->d_scalars + 16 * ctx->scalar_set; scalars_next = ctx->d_scalars + 16 * (ctx->scalar_set ^ 1);
+    }
     const bool zero_out = !(ctx->flags & CDH_FLAG_ACCUMULATE);
     const uint64_t out_count = (uint64_t)pl.n_hist * (uint64_t)pl.n_bins;
     // the repack kernel zeroes the result on its way unless that would be most of its work (few particles, very many bins)
@@ -688,8 +699,10 @@ int enqueue_plan(cdh_ctx* ctx, const Plan& pl, const void* coords, cudaStream_t 
         ++ctx->timed_calls;
     }
     for (int k = 0; k < 8; ++k) ctx->info[k] = pl.info[k];
-    if (pl.frame_slots > 0) ctx->scalar_set ^= 1;                // the repack kernel has zeroed the other set
-    ctx->scalars_dirty = false;
+    if (!capturing) {
+        if (pl.frame_slots > 0) ctx->scalar_set ^= 1;            // the repack kernel has zeroed the other set
+        ctx->scalars_dirty = false;
+    }
     return CDH_OK;
 }
 

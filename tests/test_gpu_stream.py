@@ -128,3 +128,39 @@ def test_plan_cache_many_shapes_two_streams_and_changing_coordinates():
         torch.cuda.synchronize()
         assert np.array_equal(a.cpu().numpy().view(np.uint64), cdh_oracle.problem_histograms(p, "f32"))
         assert np.array_equal(b.cpu().numpy().view(np.uint64), cdh_oracle.problem_histograms(q, "f32"))
+
+
+def test_cached_call_captured_into_a_cuda_graph_and_replayed_between_other_calls():
+    """A call that hits the plan cache enqueues kernels only (include/cdh.h): it can be recorded into a CUDA graph.  ONE captured
+    call, replayed several times with other (uncaptured) calls of the same context in between: every replay and every call in
+    between must give the oracle-checked result (the library's per-call scalars must not leak between them)."""
+    _need_gpu()
+    dev = torch.device("cuda", 0)
+    p, q = inputs.reduced_config(2), inputs.reduced_config(3)
+    want_p, want_q = cdh_oracle.problem_histograms(p, "f32"), cdh_oracle.problem_histograms(q, "f32")
+    cp, cq = torch.from_numpy(p.coords).to(dev), torch.from_numpy(q.coords).to(dev)
+    op = torch.zeros((p.n_hist, p.n_bins), dtype=torch.int64, device=dev)
+    oq = torch.zeros((q.n_hist, q.n_bins), dtype=torch.int64, device=dev)
+    s = torch.cuda.Stream()
+    with cdh.Context(0) as ctx:
+        def call(prob, coords, out):
+            ctx.cdh_histograms(coords, prob.n_frames, prob.species_offsets, prob.box_type, prob.box, prob.r_max, prob.n_bins, out, stream=s)
+        with torch.cuda.stream(s):
+            call(p, cp, op); call(q, cq, oq)            # build both plans before the capture
+        s.synchronize()
+        g = torch.cuda.CUDAGraph()
+        with torch.cuda.graph(g, stream=s):
+            call(p, cp, op)                             # one call: an odd number on purpose
+        for rep in range(3):
+            op.fill_(-1)
+            with torch.cuda.stream(s):
+                g.replay()
+            s.synchronize()
+            assert np.array_equal(op.cpu().numpy().view(np.uint64), want_p), f"replay {rep}"
+            oq.fill_(-1)
+            with torch.cuda.stream(s):
+                call(q, cq, oq)
+                if rep == 1:
+                    call(q, cq, oq)
+            s.synchronize()
+            assert np.array_equal(oq.cpu().numpy().view(np.uint64), want_q), f"uncaptured call after replay {rep}"
