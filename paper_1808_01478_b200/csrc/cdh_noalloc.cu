@@ -17,7 +17,7 @@
 // The array is shared by every call on the device and keeps the last call's contents.  What must start at zero (work
 // counter, range keys, the caller's result) is cleared by the call itself; the repacked coordinates and the tables are
 // rewritten completely.  Two calls that overlap on one GPU (different streams, different host threads) RACE on the
-// array: callers serialise them (one stream, or events).
+// array: callers serialise them (one stream, or events).  Not for recording into a CUDA graph (refused: see below).
 #include <algorithm>
 #include <cmath>
 #include <cstring>
@@ -146,6 +146,13 @@ extern "C" int cdh_histograms_noalloc(int device, const void* coords, int32_t n_
     int rc = device_setup(device, &dev);
     if (rc != CDH_OK) return rc;
     cudaStream_t stream = (cudaStream_t)stream_;
+    // The work tables go up from host memory that dies with this call: recorded into a CUDA graph, the copy would read freed
+    // memory on every replay.  Refuse instead of corrupting (a context's cached calls CAN be captured: cdh_histograms).
+    cudaStreamCaptureStatus cap = cudaStreamCaptureStatusNone;
+    NA_CUDA(cudaStreamIsCapturing(stream, &cap));
+    if (cap != cudaStreamCaptureStatusNone)
+        return fail(CDH_ERR_UNSUPPORTED, "cdh_histograms_noalloc: the stream is being captured into a CUDA graph; this entry point uploads "
+                                         "its work tables from the host on every call and cannot be replayed (cached cdh_histograms calls can)");
     unsigned char* const scratch = dev->scratch;
     unsigned int* const scalars = reinterpret_cast<unsigned int*>(scratch);
     unsigned char* const d_tables = scratch + kScalarBytes;

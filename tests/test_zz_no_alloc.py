@@ -92,3 +92,24 @@ def test_sizes_beyond_the_static_scratch_are_rejected_with_a_clear_error(dev):
     # and the entry point still works afterwards
     p = inputs.reduced_config(1)
     same(no_alloc(p, dev), existing_path(p), "config 1 after the rejected calls")
+
+
+def test_refused_on_a_capturing_stream(dev):
+    # recorded into a CUDA graph the call's table upload would read freed host memory on replay: it must refuse, record nothing,
+    # leave the capture valid, and work again afterwards
+    p = inputs.reduced_config(1)
+    coords = torch.from_numpy(p.coords).to(dev)
+    out = torch.full((p.n_hist, p.n_bins), 5, dtype=torch.int64, device=dev)
+    want = existing_path(p)
+    same(no_alloc(p, dev), want, "before the capture")          # device set-up happens outside the capture
+    s = torch.cuda.Stream()
+    g = torch.cuda.CUDAGraph()
+    with torch.cuda.graph(g, stream=s):
+        with pytest.raises(cdh.CdhError) as e:
+            cdh.cdh_histograms_noalloc(0, coords, p.n_frames, p.species_offsets, p.box_type, p.box, p.r_max, p.n_bins, out, stream=s)
+        out.add_(1)                                              # something to record, so that the graph is not empty
+    assert e.value.code == -2 and "captured" in str(e.value)
+    g.replay()
+    torch.cuda.synchronize()
+    assert int(out.min()) == 6 and int(out.max()) == 6
+    same(no_alloc(p, dev), want, "after the capture")
