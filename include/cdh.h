@@ -225,9 +225,11 @@ int cdh_rdf(cdh_ctx *ctx, const uint64_t *hist, int32_t n_hist, int32_t n_bins, 
  * padded to a multiple of 4096 particles; n_bins <= CDH_NOALLOC_MAX_BINS; work tables (48 B per frame and species
  * pair + 16 B per i-tile of 1,024 or 4,096 particles + 560 B per box) <= 255.75 KiB.  Larger problems: cdh_histograms.
  * The array is SHARED by all calls on a device and keeps the last call's contents; the call clears what must start
- * at zero.  Calls that overlap on one GPU (two streams, two host threads) race on it: serialise them.  The call cannot be
- * RECORDED into a CUDA graph (its work tables are copied from host memory of the call): on a capturing stream it returns
- * CDH_ERR_UNSUPPORTED and records nothing; cached cdh_histograms calls can be recorded.
+ * at zero.  Calls that overlap on one GPU (two streams, two host threads) race on it: serialise them.  RECORDING into a
+ * CUDA graph: a call whose work tables are at most 32,000 bytes (they then travel as a kernel parameter: 3 species x about
+ * 100 frames, or a single frame of any size the scratch holds) reads no host memory on the device and can be recorded and
+ * replayed, provided the entry point was called once on the device before the capture; with larger tables (copied from
+ * host memory of the call) it returns CDH_ERR_UNSUPPORTED on a capturing stream and records nothing.
  * Returns CDH_OK, CDH_ERR_INVALID_ARG, CDH_ERR_UNSUPPORTED or CDH_ERR_CUDA; text via cdh_noalloc_last_error()
  * (per host thread, valid until that thread's next call).
  */

@@ -17,7 +17,9 @@
 // The array is shared by every call on the device and keeps the last call's contents.  What must start at zero (work
 // counter, range keys, the caller's result) is cleared by the call itself; the repacked coordinates and the tables are
 // rewritten completely.  Two calls that overlap on one GPU (different streams, different host threads) RACE on the
-// array: callers serialise them (one stream, or events).  Not for recording into a CUDA graph (refused: see below).
+// array: callers serialise them (one stream, or events).  Recording into a CUDA graph: calls whose work tables fit a kernel
+// parameter (32,000 bytes: e.g. 3 species x 100 frames, or one frame of any size the scratch holds) have no node that reads
+// host memory and can be replayed; larger ones are refused on a capturing stream.
 #include <algorithm>
 #include <cmath>
 #include <cstring>
@@ -88,6 +90,26 @@ int device_setup(int device, DeviceSetup** out) {
 
 inline size_t align256(size_t x) { return (x + 255) & ~(size_t)255; }
 
+// Small work tables travel as a kernel PARAMETER (copied by value when the launch is enqueued or recorded), not as a copy from
+// host memory: the call then has no node that reads the host, and can be recorded into a CUDA graph and replayed.
+template <int N16>
+struct alignas(16) TableBlob { uint4 q[N16]; };
+constexpr int kBlobSmall = 250, kBlobLarge = 2000;            // 4,000 and 32,000 bytes (kernel parameters: up to 32,764 bytes)
+
+template <int N16>
+__global__ void __launch_bounds__(256) tables_from_params(const __grid_constant__ TableBlob<N16> blob, uint4* dst, uint32_t n16) {
+    for (uint32_t k = blockIdx.x * 256u + threadIdx.x; k < n16; k += gridDim.x * 256u) dst[k] = blob.q[k];
+}
+
+template <int N16>
+cudaError_t upload_by_value(const unsigned char* h, size_t bytes, unsigned char* dst, cudaStream_t stream) {
+    static thread_local TableBlob<N16> blob;                   // host staging of the parameter (static: no allocation per call)
+    std::memcpy(blob.q, h, bytes);
+    const uint32_t n16 = (uint32_t)((bytes + 15) / 16);
+    tables_from_params<N16><<<(n16 + 255) / 256, 256, 0, stream>>>(blob, reinterpret_cast<uint4*>(dst), n16);
+    return cudaGetLastError();
+}
+
 }  // namespace
 
 extern "C" const char* cdh_noalloc_last_error(void) { return t_err.c_str(); }
@@ -146,13 +168,9 @@ extern "C" int cdh_histograms_noalloc(int device, const void* coords, int32_t n_
     int rc = device_setup(device, &dev);
     if (rc != CDH_OK) return rc;
     cudaStream_t stream = (cudaStream_t)stream_;
-    // The work tables go up from host memory that dies with this call: recorded into a CUDA graph, the copy would read freed
-    // memory on every replay.  Refuse instead of corrupting (a context's cached calls CAN be captured: cdh_histograms).
     cudaStreamCaptureStatus cap = cudaStreamCaptureStatusNone;
     NA_CUDA(cudaStreamIsCapturing(stream, &cap));
-    if (cap != cudaStreamCaptureStatusNone)
-        return fail(CDH_ERR_UNSUPPORTED, "cdh_histograms_noalloc: the stream is being captured into a CUDA graph; this entry point uploads "
-                                         "its work tables from the host on every call and cannot be replayed (cached cdh_histograms calls can)");
+    const bool capturing = cap != cudaStreamCaptureStatusNone;     // the call is being recorded into a CUDA graph
     unsigned char* const scratch = dev->scratch;
     unsigned int* const scalars = reinterpret_cast<unsigned int*>(scratch);
     unsigned char* const d_tables = scratch + kScalarBytes;
@@ -195,7 +213,13 @@ extern "C" int cdh_histograms_noalloc(int device, const void* coords, int32_t n_
         return fail(CDH_ERR_UNSUPPORTED, "cdh_histograms_noalloc: the work tables of the call (" + std::to_string(tables) +
                                              " bytes: frames x species pairs x i-tiles) exceed the maximum of " + std::to_string(kTableBytes) +
                                              " bytes: use cdh_histograms");
-    std::vector<unsigned char> h(tables, 0);
+    // Larger tables are copied from host memory that dies with this call: recorded into a graph, that copy would read freed
+    // memory on every replay.  Refuse instead of corrupting.
+    if (capturing && tables > (size_t)kBlobLarge * 16)
+        return fail(CDH_ERR_UNSUPPORTED, "cdh_histograms_noalloc: the stream is being captured into a CUDA graph and the work tables of the call (" +
+                                             std::to_string(tables) + " bytes) exceed the " + std::to_string(kBlobLarge * 16) +
+                                             " bytes that travel as a kernel parameter; this call cannot be replayed (cached cdh_histograms calls can)");
+    std::vector<unsigned char> h(align256(tables) + 16, 0);
     std::memcpy(h.data(), wt.segs.data(), wt.segs.size() * sizeof(Seg));
     std::memcpy(h.data() + o_rows, wt.rows.data(), wt.rows.size() * sizeof(Row));
     std::memcpy(h.data() + o_boxes, boxes.data(), n_box_rec * sizeof(BoxConst));
@@ -206,7 +230,9 @@ extern "C" int cdh_histograms_noalloc(int device, const void* coords, int32_t n_
     NA_CUDA(cudaMemsetAsync(scalars, 0, 128, stream));                               // work counter, range keys
     NA_CUDA(cudaMemsetAsync(out, 0, out_count * sizeof(uint64_t), stream));          // the caller's result is overwritten
     if (frame_slots == 0) return CDH_OK;
-    NA_CUDA(cudaMemcpyAsync(d_tables, h.data(), tables, cudaMemcpyHostToDevice, stream));   // pageable: staged before the call returns
+    if (tables <= (size_t)kBlobSmall * 16) NA_CUDA(upload_by_value<kBlobSmall>(h.data(), tables, d_tables, stream));
+    else if (tables <= (size_t)kBlobLarge * 16) NA_CUDA(upload_by_value<kBlobLarge>(h.data(), tables, d_tables, stream));
+    else NA_CUDA(cudaMemcpyAsync(d_tables, h.data(), tables, cudaMemcpyHostToDevice, stream));   // pageable: staged before the call returns
     RepackParams rp;
     rp.coords = (const float*)coords; rp.pk = d_pk;
     rp.off = (const int32_t*)(d_tables + o_off); rp.pad_off = (const uint32_t*)(d_tables + o_pad);

@@ -94,14 +94,38 @@ def test_sizes_beyond_the_static_scratch_are_rejected_with_a_clear_error(dev):
     same(no_alloc(p, dev), existing_path(p), "config 1 after the rejected calls")
 
 
-def test_refused_on_a_capturing_stream(dev):
-    # recorded into a CUDA graph the call's table upload would read freed host memory on replay: it must refuse, record nothing,
-    # leave the capture valid, and work again afterwards
-    p = inputs.reduced_config(1)
+def test_recorded_into_a_cuda_graph_and_replayed(dev):
+    """Calls with small work tables (they travel as a kernel parameter) have no node that reads host memory: recorded into a
+    CUDA graph and replayed, with OTHER calls of the entry point in between (which overwrite the shared scratch), every replay
+    must rebuild everything it needs and give the existing path's result."""
+    p, q = inputs.reduced_config(2), inputs.reduced_config(3)
+    want_p, want_q = existing_path(p), existing_path(q)
+    same(no_alloc(p, dev), want_p, "before the capture")        # device set-up (cudaGetSymbolAddress) happens outside the capture
+    coords = torch.from_numpy(p.coords).to(dev)
+    out = torch.empty((p.n_hist, p.n_bins), dtype=torch.int64, device=dev)
+    s = torch.cuda.Stream()
+    g = torch.cuda.CUDAGraph()
+    with torch.cuda.graph(g, stream=s):
+        cdh.cdh_histograms_noalloc(0, coords, p.n_frames, p.species_offsets, p.box_type, p.box, p.r_max, p.n_bins, out, stream=s)
+    for rep in range(3):
+        out.fill_(-3)
+        with torch.cuda.stream(s):
+            g.replay()
+        s.synchronize()
+        same(out.cpu().numpy().view(np.uint64), want_p, f"replay {rep}")
+        same(no_alloc(q, dev, stream=s), want_q, f"another problem through the same scratch after replay {rep}")
+
+
+def test_large_tables_are_refused_on_a_capturing_stream(dev):
+    # 32 species: 528 species pairs, 33.8 KB of work tables -- more than a kernel parameter holds, so they are copied from host
+    # memory of the call; recorded into a graph that copy would read freed memory on replay: the call must refuse, record
+    # nothing, leave the capture valid, and work again afterwards
+    counts = (3,) * 32
+    p = inputs.uniform_problem(99, counts, inputs.BOX_NONE, 50, 2.0)
     coords = torch.from_numpy(p.coords).to(dev)
     out = torch.full((p.n_hist, p.n_bins), 5, dtype=torch.int64, device=dev)
     want = existing_path(p)
-    same(no_alloc(p, dev), want, "before the capture")          # device set-up happens outside the capture
+    same(no_alloc(p, dev), want, "32 species, not captured")
     s = torch.cuda.Stream()
     g = torch.cuda.CUDAGraph()
     with torch.cuda.graph(g, stream=s):
