@@ -87,7 +87,7 @@ __global__ void __launch_bounds__(T, MINB) tile_kernel(const typename M::Params 
     // fetches item k + 1 WHILE item k is computed: the counter value it needs was requested one item earlier (the atomic
     // is not waited for until then), and the descriptor travels from the plan's table into the other of two shared-memory
     // slots as an asynchronous copy, so nothing but one CTA barrier stands between two items (the serial chain atomic ->
-    // row search -> Row -> Seg of the first version cost configs 2-4 1.5-2 %).  Calls with more items than the table holds
+    // row search -> Row -> Seg of the first version cost configs 2, 4 and 5 2-4 %).  Calls with more items than the table holds
     // look the next item up with ordinary loads at the same point (thread 0's warp then lags by those round trips).
     // A slot whose index field says kNoItem ends the CTA's loop.
     constexpr uint32_t kNoItem = 0xFFFFFFFFu;
@@ -137,7 +137,7 @@ __global__ void __launch_bounds__(T, MINB) tile_kernel(const typename M::Params 
     const bool one_each = gridDim.x >= P.n_items;      // one CTA per item (small calls): the counter is never touched
     // Claiming an item one item early costs balance at the end of a launch that gives a CTA only a few items (a CTA holds
     // an item it will not start for a while; 10,000 points, 2 items per CTA: 986 Gpairs/s claiming ahead, 1,146 claiming
-    // late).  The run-time choice is compiled into the SKIP kernels only -- the ones single frames of small species run --
+    // late).  The run-time choice is compiled into the SKIP kernels only -- the ones few-item calls and small species run --
     // because the second code path costs the large-problem kernels 1.0-1.7 % (another ptxas schedule of the pair loops).
     const bool ahead = !SKIP || P.claim_ahead != 0u;
     uint32_t nxt = 0;                                  // thread 0: the counter value that numbers the item to fetch next
