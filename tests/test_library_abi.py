@@ -55,6 +55,14 @@ def test_null_arguments_are_rejected_without_a_device(lib):
     assert lib.cdh_destroy(None) == binding.OK
     info = (ctypes.c_int64 * 8)()
     assert lib.cdh_last_call_info(None, info) == binding.ERR_INVALID_ARG
+    # the entry point without a context checks its arguments, and its size limits, before it touches a device
+    assert lib.cdh_histograms_noalloc(0, None, 1, off.ctypes.data, 1, 0, None, 0, 1.0, 8, None, 1) == binding.ERR_INVALID_ARG
+    assert b"null pointer" in lib.cdh_noalloc_last_error()
+    big = np.array([0, 131073], dtype=np.int32)
+    assert lib.cdh_histograms_noalloc(0, 1, 1, big.ctypes.data, 1, 0, None, 0, 1.0, 8, None, 1) == binding.ERR_UNSUPPORTED
+    assert b"131072 padded particles" in lib.cdh_noalloc_last_error()
+    assert lib.cdh_histograms_noalloc(0, 1, 1, off.ctypes.data, 1, 0, None, 0, 1.0, 32769, None, 1) == binding.ERR_UNSUPPORTED
+    assert b"n_bins" in lib.cdh_noalloc_last_error()
 
 
 def test_no_cpu_fallback_when_library_is_missing(tmp_path):
